@@ -1,0 +1,133 @@
+/* mg.h -- C-ABI of libmg: masked rasterization of 3D Gaussians (MaskGaussian, arXiv 2412.20522)
+ * for NVIDIA B200 (sm_100a).  Citations "PAPER.md:n" are lines of the paper text; "reading k" is a
+ * row of DESIGN.md's table of readings (where the paper is silent).
+ *
+ * One training-iteration pass of the hot path is five calls, in this order:
+ *
+ *   mg_preprocess      splat every Gaussian, masks NOT consulted  (PAPER.md:64-66 sec. 3.1; :30, :78)
+ *   mg_bin_sort        per-tile depth-ordered lists                (PAPER.md:66 "depth order"; :74 16x16 tiles)
+ *   mg_render_fwd      masked blend, Eq. 3-4 + background Eq. 9-10
+ *   mg_render_bwd      reverse traversal, Eq. 11-18 -> dL/dM_i and the usual gradients
+ *   mg_preprocess_bwd  chain rule through the projection           (implied by PAPER.md:156)
+ *
+ * Conventions
+ *   - Every call returns 0 (MG_OK) or a negative mg_status; mg_last_error_string() describes the last
+ *     failure on the calling thread.  No exceptions cross the boundary.
+ *   - Every array pointer is a DEVICE pointer unless its name ends in _host (pinned or pageable HOST
+ *     memory written asynchronously: valid after the stream is synchronised).  `cam` is a HOST pointer,
+ *     read during the call.  The caller owns every buffer; the library allocates nothing persistent.
+ *   - `stream` is a cudaStream_t (NULL = default stream).  All work is enqueued on it; calls are
+ *     asynchronous.
+ *   - Layouts: packed row-major fp32.  means[N][3], log_scales[N][3], quats[N][4] as (w,x,y,z),
+ *     opacity_logits[N], sh[N][K][3] with K=(sh_degree+1)^2 (coefficient-major, RGB innermost),
+ *     masks[N] (any real value; tests use {0,1}; Eq. 4 is affine in M), images planar [3][H][W].
+ *     Float arrays must be 16-byte aligned (cudaMalloc / torch allocations are).
+ *   - Gradient outputs are OVERWRITTEN (never accumulated into caller content).  Culled Gaussians get
+ *     exact zeros everywhere, including dL_dmask.
+ */
+#ifndef MG_H_
+#define MG_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Constants of the method (readings 1, 11-14; the paper states none of them). */
+#define MG_TILE 16              /* PAPER.md:74 "tile (16x16 grid)" */
+#define MG_ALPHA_MIN (1.0f / 255.0f) /* a pair with alpha < 1/255 is skipped (mask not consulted) */
+#define MG_ALPHA_MAX 0.99f      /* alpha = min(0.99, o * G) */
+#define MG_T_MIN 1e-4f          /* a pixel stops before the entry that would take T below 1e-4 */
+#define MG_DILATION 0.3f        /* low-pass added to the diagonal of the 2D covariance */
+#define MG_ZNEAR 0.2f           /* Gaussians with camera-space z <= 0.2 are culled */
+#define MG_JCLAMP 1.3f          /* x/z, y/z clamped to +-1.3*W/(2fx), +-1.3*H/(2fy) inside the Jacobian */
+#define MG_EIG_FLOOR 0.1f       /* floor under the square root of the eigenvalue formula */
+
+typedef enum {
+  MG_OK = 0,
+  MG_ERR_INVALID_ARG = -1, /* null pointer, negative size, sh_degree outside 0..3, image larger than 2^15 tiles per side */
+  MG_ERR_CAPACITY = -2,    /* caller buffer or workspace too small */
+  MG_ERR_CUDA = -3         /* a CUDA call failed; see mg_last_error_string() */
+} mg_status;
+
+typedef struct {
+  int32_t width, height;
+  float fx, fy, cx, cy; /* pinhole intrinsics in pixels; pixel (i,j) has its centre at (i+0.5, j+0.5) (reading 15) */
+  float R[9];           /* world->camera rotation, row-major: x_cam = R x_world + t; camera looks down +z, x right, y down */
+  float t[3];
+  float bg[3];          /* background colour c_bg (Eq. 10) */
+  int32_t sh_degree;    /* 0..3 */
+} mg_camera;
+
+const char* mg_last_error_string(void);
+int mg_version(void);
+
+/* Bytes of device scratch mg_bin_sort needs for N Gaussians, a width x height image and at most
+ * R_capacity duplicated keys.  Returns 0 on invalid arguments. */
+size_t mg_workspace_bytes(int64_t N, int32_t width, int32_t height, uint64_t R_capacity);
+
+/* Step a1-a3.  Per Gaussian: s = exp(log_scale), q/|q|, o = sigmoid(logit);
+ * camera-space mean, cull z <= MG_ZNEAR; Sigma = Rot S^2 Rot^T; Sigma2D = J W Sigma W^T J^T + 0.3 I;
+ * conic = Sigma2D^-1; projected centre; colour = max(0, 0.5 + sum_j Y_j(dir) sh_j); radius =
+ * ceil(3 sqrt(lambda_max)); rectangle of 16x16 tiles touched.  Masks are not an argument: "all
+ * Gaussians are splatted without any attribute masked out".
+ * Outputs (culled Gaussians: zeros, radii = 0, tiles_touched = 0):
+ *   means2d[N][2] pixel-index coordinates; depths[N] camera z; conic_opacity[N][4] = (A, B, C, o) with
+ *   power = -1/2 (A dx^2 + 2 B dx dy + C dy^2); rgb[N][3]; radii[N]; rects[N][4] = (x0, y0, x1, y1) in
+ *   tile units, max exclusive; tiles_touched[N]; clamped[N] bit k = colour channel k clamped at 0.
+ *   num_rendered_host (may be NULL): sum of tiles_touched = R, written asynchronously. */
+int mg_preprocess(const mg_camera* cam, int64_t N, const float* means, const float* log_scales, const float* quats,
+                  const float* opacity_logits, const float* sh, float* means2d, float* depths, float* conic_opacity,
+                  float* rgb, int32_t* radii, int32_t* rects, uint32_t* tiles_touched, uint8_t* clamped,
+                  uint64_t* num_rendered_host, void* stream);
+
+/* Step a4-a6.  Result = the duplicated (tile, depth) keys in ascending order of the
+ * 64-bit key (tile_id << 32 | fp32 bits of depth), ties by Gaussian index, tile_id = ty * gw + tx:
+ *   sorted_ids[R]       Gaussian index of each sorted key
+ *   tile_ranges[gw*gh][2] = [start, end) of each tile in sorted_ids (start == end for an empty tile)
+ *   R_out_host (may be NULL): the true R, written asynchronously.
+ * R must be < 2^32.  If R > R_capacity nothing is written to sorted_ids, every tile range is set to
+ * [0, 0) and *R_out_host (> R_capacity) tells the caller to retry with larger buffers.
+ * workspace: at least mg_workspace_bytes(N, W, H, R_capacity) bytes, 256-byte aligned. */
+int mg_bin_sort(const mg_camera* cam, int64_t N, const float* depths, const int32_t* rects,
+                const uint32_t* tiles_touched, uint64_t R_capacity, void* workspace, size_t workspace_bytes,
+                uint32_t* sorted_ids, uint32_t* tile_ranges, uint64_t* R_out_host, void* stream);
+
+/* Step a7 (Eq. 3-4; Eq. 9-10).  Per pixel, front to back over its tile's
+ * list: alpha = min(0.99, o G); skip if power > 0 or alpha < 1/255 (mask NOT consulted, reading 2);
+ * a = M alpha; T' = T (1 - a); stop if T' < 1e-4 (this entry is not blended, reading 3-4);
+ * C += a T c; T = T'.  Then image = C + T c_bg.
+ *   image[3][H][W]; final_T[H][W] = T_{N+1}; n_contrib[H][W] = 1-based list position of the last entry
+ *   that was blended, masked or not (0 if none; reading 5). */
+int mg_render_fwd(const mg_camera* cam, const uint32_t* sorted_ids, const uint32_t* tile_ranges,
+                  const float* means2d, const float* conic_opacity, const float* rgb, const float* masks,
+                  float* image, float* final_T, uint32_t* n_contrib, void* stream);
+
+/* Step a8 (Eq. 11, 13-18).  Per pixel, from its last contributor back to the front:
+ * T_i = T_{i+1} / (1 - a_i); b by the recursion of Eq. 11; dL/dM_i by Eq. 18 (including the background
+ * term); dL/dalpha_i = M_i * (same bracket); chain to colour, opacity (w.r.t. the activated o), conic and
+ * projected centre (pixels).  Zero gradient to (o, conic, centre) where the 0.99 clamp is active
+ * (reading 6).  A masked Gaussian (M = 0) gets dL/dM only (Fig. 1).
+ * Sums over pixels use fp32 atomics: results vary in the last bits from run to run. */
+int mg_render_bwd(const mg_camera* cam, int64_t N, const uint32_t* sorted_ids, const uint32_t* tile_ranges,
+                  const float* means2d, const float* conic_opacity, const float* rgb, const float* masks,
+                  const float* final_T, const uint32_t* n_contrib, const float* dL_dimage, float* dL_dmeans2d,
+                  float* dL_dconic, float* dL_dopacity, float* dL_drgb, float* dL_dmask, void* stream);
+
+/* Step a9.  Vector-Jacobian product of mg_preprocess: from (dL_dmeans2d[N][2], dL_dconic[N][3] for
+ * (A,B,C), dL_dopacity[N], dL_drgb[N][3]) to gradients w.r.t. the raw inputs: dL_dmeans[N][3],
+ * dL_dlog_scales[N][3], dL_dquats[N][4] (w.r.t. the un-normalised quaternion), dL_dopacity_logits[N],
+ * dL_dsh[N][K][3].  No gradient flows through depth, radius or rect; none through a clamped colour
+ * channel.  radii and clamped are mg_preprocess's outputs for the same inputs and camera. */
+int mg_preprocess_bwd(const mg_camera* cam, int64_t N, const float* means, const float* log_scales,
+                      const float* quats, const float* opacity_logits, const float* sh, const int32_t* radii,
+                      const uint8_t* clamped, const float* dL_dmeans2d, const float* dL_dconic,
+                      const float* dL_dopacity, const float* dL_drgb, float* dL_dmeans, float* dL_dlog_scales,
+                      float* dL_dquats, float* dL_dopacity_logits, float* dL_dsh, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MG_H_ */

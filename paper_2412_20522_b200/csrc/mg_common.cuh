@@ -1,0 +1,55 @@
+// mg_common.cuh -- shared by the kernels of libmg (product code; nothing here is used by oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "mg.h"
+
+void mg_set_error(const char* fmt, ...);
+
+#define MG_CHECK_CUDA(expr)                                                              \
+  do {                                                                                   \
+    cudaError_t e__ = (expr);                                                            \
+    if (e__ != cudaSuccess) {                                                            \
+      mg_set_error("%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e__), __FILE__, __LINE__); \
+      return MG_ERR_CUDA;                                                                \
+    }                                                                                    \
+  } while (0)
+
+#define MG_CHECK_LAUNCH() MG_CHECK_CUDA(cudaGetLastError())
+
+#define MG_REQUIRE(cond, msg)               \
+  do {                                      \
+    if (!(cond)) {                          \
+      mg_set_error("invalid argument: %s", msg); \
+      return MG_ERR_INVALID_ARG;            \
+    }                                       \
+  } while (0)
+
+static inline int mg_check_camera(const mg_camera* cam) {
+  MG_REQUIRE(cam != nullptr, "cam is null");
+  MG_REQUIRE(cam->width > 0 && cam->height > 0, "image size must be positive");
+  MG_REQUIRE(cam->width <= (1 << 19) && cam->height <= (1 << 19), "image larger than 2^15 tiles per side");
+  MG_REQUIRE(cam->sh_degree >= 0 && cam->sh_degree <= 3, "sh_degree must be 0..3");
+  MG_REQUIRE(cam->fx > 0.f && cam->fy > 0.f, "focal lengths must be positive");
+  return MG_OK;
+}
+
+static inline int mg_grid_w(const mg_camera* c) { return (c->width + MG_TILE - 1) / MG_TILE; }
+static inline int mg_grid_h(const mg_camera* c) { return (c->height + MG_TILE - 1) / MG_TILE; }
+
+// Real spherical-harmonics constants (Condon-Shortley sign, order l, m=-l..l; reading 16).
+#define MG_SH_C0 0.28209479177387814f
+#define MG_SH_C1 0.4886025119029199f
+#define MG_SH_C2_0 1.0925484305920792f
+#define MG_SH_C2_1 -1.0925484305920792f
+#define MG_SH_C2_2 0.31539156525252005f
+#define MG_SH_C2_3 -1.0925484305920792f
+#define MG_SH_C2_4 0.5462742152960396f
+#define MG_SH_C3_0 -0.5900435899266435f
+#define MG_SH_C3_1 2.890611442640554f
+#define MG_SH_C3_2 -0.4570457994644658f
+#define MG_SH_C3_3 0.3731763325901154f
+#define MG_SH_C3_4 -0.4570457994644658f
+#define MG_SH_C3_5 1.445305721320277f
+#define MG_SH_C3_6 -0.5900435899266435f

