@@ -93,18 +93,23 @@ __global__ void __launch_bounds__(256) preprocess_kernel(
       const float T10 = J11 * R[3] + J12 * R[6], T11 = J11 * R[4] + J12 * R[7], T12 = J11 * R[5] + J12 * R[8];
       const float U00 = T00 * M00 + T01 * M10 + T02 * M20, U01 = T00 * M01 + T01 * M11 + T02 * M21, U02 = T00 * M02 + T01 * M12 + T02 * M22;
       const float U10 = T10 * M00 + T11 * M10 + T12 * M20, U11 = T10 * M01 + T11 * M11 + T12 * M21, U12 = T10 * M02 + T11 * M12 + T12 * M22;
-      const float a = U00 * U00 + U01 * U01 + U02 * U02 + MG_DILATION;
+      const float n0 = U00 * U00 + U01 * U01 + U02 * U02, n1 = U10 * U10 + U11 * U11 + U12 * U12;
+      const float a = n0 + MG_DILATION;
       const float b = U00 * U10 + U01 * U11 + U02 * U12;
-      const float c = U10 * U10 + U11 * U11 + U12 * U12 + MG_DILATION;
-      // O5 conic
-      const float det = a * c - b * b;
+      const float c = n1 + MG_DILATION;
+      // O5 conic.  det(U U^T + h I) = |U0 x U1|^2 + h (|U0|^2 + |U1|^2) + h^2: the same number as
+      // a c - b^2 (Lagrange's identity) but a sum of non-negative terms, so fp32 keeps its relative
+      // accuracy for elongated splats where a c and b^2 nearly cancel.
+      const float cx = U01 * U12 - U02 * U11, cy = U02 * U10 - U00 * U12, cz = U00 * U11 - U01 * U10;
+      const float det = (cx * cx + cy * cy + cz * cz) + MG_DILATION * (n0 + n1) + MG_DILATION * MG_DILATION;
       if (det > 0.f) {
         const float idet = 1.f / det;
         // O6 centre in pixel-index coordinates
         const float mx = cam.fx * tx * iz + (cam.cx - 0.5f), my = cam.fy * ty * iz + (cam.cy - 0.5f);
         // O7 radius and tile rectangle
         const float mid = 0.5f * (a + c);
-        const float lam = mid + sqrtf(fmaxf(mid * mid - det, MG_EIG_FLOOR));
+        const float hd = 0.5f * (a - c);
+        const float lam = mid + sqrtf(fmaxf(hd * hd + b * b, MG_EIG_FLOOR));  // mid^2 - det = ((a-c)/2)^2 + b^2
         const float rad_f = ceilf(3.f * sqrtf(lam));
         const int gw = (cam.width + MG_TILE - 1) / MG_TILE, gh = (cam.height + MG_TILE - 1) / MG_TILE;
         const float inv_tile = 1.f / MG_TILE;

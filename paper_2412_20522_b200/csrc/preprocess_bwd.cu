@@ -36,7 +36,7 @@ __global__ void __launch_bounds__(128) preprocess_bwd_kernel(
   const float* R = cam.R;
   const float px = means[3 * i], py = means[3 * i + 1], pz = means[3 * i + 2];
   const float4 q = __ldg(reinterpret_cast<const float4*>(quats) + i);
-  const float s0 = expf(log_scales[3 * i]), s1 = expf(log_scales[3 * i + 1]), s2 = expf(log_scales[3 * i + 2]);
+  const double s0 = exp((double)log_scales[3 * i]), s1 = exp((double)log_scales[3 * i + 1]), s2 = exp((double)log_scales[3 * i + 2]);
   const float o = 1.f / (1.f + expf(-opacity_logits[i]));
   const float2 gm = dL_dmeans2d[i];
   const float gA = dL_dconic[3 * i], gB = dL_dconic[3 * i + 1], gC = dL_dconic[3 * i + 2];
@@ -111,88 +111,104 @@ __global__ void __launch_bounds__(128) preprocess_bwd_kernel(
     }
   }
 
-  // ---------------- geometry: recompute the forward quantities ----------------
-  const float tx = R[0] * px + R[1] * py + R[2] * pz + cam.t[0];
-  const float ty = R[3] * px + R[4] * py + R[5] * pz + cam.t[1];
-  const float tz = R[6] * px + R[7] * py + R[8] * pz + cam.t[2];
-  const float qn2 = q.x * q.x + q.y * q.y + q.z * q.z + q.w * q.w;
-  const float qinv = rsqrtf(qn2);
-  const float qw = q.x * qinv, qx = q.y * qinv, qy = q.z * qinv, qz = q.w * qinv;
-  const float r00 = 1.f - 2.f * (qy * qy + qz * qz), r01 = 2.f * (qx * qy - qw * qz), r02 = 2.f * (qx * qz + qw * qy);
-  const float r10 = 2.f * (qx * qy + qw * qz), r11 = 1.f - 2.f * (qx * qx + qz * qz), r12 = 2.f * (qy * qz - qw * qx);
-  const float r20 = 2.f * (qx * qz - qw * qy), r21 = 2.f * (qy * qz + qw * qx), r22 = 1.f - 2.f * (qx * qx + qy * qy);
-  const float M00 = r00 * s0, M01 = r01 * s1, M02 = r02 * s2;
-  const float M10 = r10 * s0, M11 = r11 * s1, M12 = r12 * s2;
-  const float M20 = r20 * s0, M21 = r21 * s1, M22 = r22 * s2;
-  const float limx = MG_JCLAMP * cam.width / (2.f * cam.fx), limy = MG_JCLAMP * cam.height / (2.f * cam.fy);
-  const float iz = 1.f / tz;
-  const float xz_raw = tx * iz, yz_raw = ty * iz;
+  // ---------------- geometry, in fp64 ----------------
+  // dL/dconic is a sum of q d d^T over pixels; mapping it back through conic = Sigma2D^-1 contracts it
+  // with vectors (A,B).d that are small for d along the major axis of an elongated splat, so the three
+  // products cancel to ~(k2/k1)^2 of their size.  fp32 loses up to 1e-3 of dL/dlog_scale there; this
+  // kernel is HBM-bound and ~300 fp64 flops per Gaussian are free, so the geometry chain runs in fp64
+  // on the fp32 inputs and is rounded once at the end.
+  typedef double G;
+  G Rd[9], td[3];
+#pragma unroll
+  for (int j = 0; j < 9; j++) Rd[j] = (G)cam.R[j];
+#pragma unroll
+  for (int j = 0; j < 3; j++) td[j] = (G)cam.t[j];
+  const G fxd = (G)cam.fx, fyd = (G)cam.fy;
+  const G pxd = px, pyd = py, pzd = pz;
+  const G tx = Rd[0] * pxd + Rd[1] * pyd + Rd[2] * pzd + td[0];
+  const G ty = Rd[3] * pxd + Rd[4] * pyd + Rd[5] * pzd + td[1];
+  const G tz = Rd[6] * pxd + Rd[7] * pyd + Rd[8] * pzd + td[2];
+  const G qn2 = (G)q.x * q.x + (G)q.y * q.y + (G)q.z * q.z + (G)q.w * q.w;
+  const G qinv = (G)1 / sqrt(qn2);
+  const G qw = q.x * qinv, qx = q.y * qinv, qy = q.z * qinv, qz = q.w * qinv;
+  const G r00 = (G)1. - (G)2. * (qy * qy + qz * qz), r01 = (G)2. * (qx * qy - qw * qz), r02 = (G)2. * (qx * qz + qw * qy);
+  const G r10 = (G)2. * (qx * qy + qw * qz), r11 = (G)1. - (G)2. * (qx * qx + qz * qz), r12 = (G)2. * (qy * qz - qw * qx);
+  const G r20 = (G)2. * (qx * qz - qw * qy), r21 = (G)2. * (qy * qz + qw * qx), r22 = (G)1. - (G)2. * (qx * qx + qy * qy);
+  const G M00 = r00 * s0, M01 = r01 * s1, M02 = r02 * s2;
+  const G M10 = r10 * s0, M11 = r11 * s1, M12 = r12 * s2;
+  const G M20 = r20 * s0, M21 = r21 * s1, M22 = r22 * s2;
+  const G limx = (G)MG_JCLAMP * cam.width / ((G)2. * fxd), limy = (G)MG_JCLAMP * cam.height / ((G)2. * fyd);
+  const G iz = (G)1. / tz;
+  const G xz_raw = tx * iz, yz_raw = ty * iz;
   const bool xcl = xz_raw < -limx || xz_raw > limx, ycl = yz_raw < -limy || yz_raw > limy;
-  const float xz = fminf(limx, fmaxf(-limx, xz_raw)), yz = fminf(limy, fmaxf(-limy, yz_raw));
-  const float J00 = cam.fx * iz, J02 = -cam.fx * xz * iz, J11 = cam.fy * iz, J12 = -cam.fy * yz * iz;
-  const float T00 = J00 * R[0] + J02 * R[6], T01 = J00 * R[1] + J02 * R[7], T02 = J00 * R[2] + J02 * R[8];
-  const float T10 = J11 * R[3] + J12 * R[6], T11 = J11 * R[4] + J12 * R[7], T12 = J11 * R[5] + J12 * R[8];
-  const float U00 = T00 * M00 + T01 * M10 + T02 * M20, U01 = T00 * M01 + T01 * M11 + T02 * M21, U02 = T00 * M02 + T01 * M12 + T02 * M22;
-  const float U10 = T10 * M00 + T11 * M10 + T12 * M20, U11 = T10 * M01 + T11 * M11 + T12 * M21, U12 = T10 * M02 + T11 * M12 + T12 * M22;
-  const float a = U00 * U00 + U01 * U01 + U02 * U02 + MG_DILATION;
-  const float b = U00 * U10 + U01 * U11 + U02 * U12;
-  const float c = U10 * U10 + U11 * U11 + U12 * U12 + MG_DILATION;
-  const float det = a * c - b * b;
-  const float idet = 1.f / det, idet2 = idet * idet;
+  const G xz = fmin(limx, fmax(-limx, xz_raw)), yz = fmin(limy, fmax(-limy, yz_raw));
+  const G J00 = fxd * iz, J02 = -fxd * xz * iz, J11 = fyd * iz, J12 = -fyd * yz * iz;
+  const G T00 = J00 * Rd[0] + J02 * Rd[6], T01 = J00 * Rd[1] + J02 * Rd[7], T02 = J00 * Rd[2] + J02 * Rd[8];
+  const G T10 = J11 * Rd[3] + J12 * Rd[6], T11 = J11 * Rd[4] + J12 * Rd[7], T12 = J11 * Rd[5] + J12 * Rd[8];
+  const G U00 = T00 * M00 + T01 * M10 + T02 * M20, U01 = T00 * M01 + T01 * M11 + T02 * M21, U02 = T00 * M02 + T01 * M12 + T02 * M22;
+  const G U10 = T10 * M00 + T11 * M10 + T12 * M20, U11 = T10 * M01 + T11 * M11 + T12 * M21, U12 = T10 * M02 + T11 * M12 + T12 * M22;
+  const G n0 = U00 * U00 + U01 * U01 + U02 * U02, n1 = U10 * U10 + U11 * U11 + U12 * U12;
+  const G a = n0 + (G)MG_DILATION;
+  const G b = U00 * U10 + U01 * U11 + U02 * U12;
+  const G c = n1 + (G)MG_DILATION;
+  // det = a c - b^2 as a sum of non-negative terms (see preprocess.cu)
+  const G crx = U01 * U12 - U02 * U11, cry = U02 * U10 - U00 * U12, crz = U00 * U11 - U01 * U10;
+  const G det = (crx * crx + cry * cry + crz * crz) + (G)MG_DILATION * (n0 + n1) + (G)MG_DILATION * (G)MG_DILATION;
+  const G idet = (G)1. / det, idet2 = idet * idet;
 
   // ---------------- reverse ----------------
   // conic (A,B,C) = (c,-b,a)/det  ->  covariance (a,b,c)
-  const float da = idet2 * (-c * c * gA + b * c * gB - b * b * gC);
-  const float db = idet2 * (2.f * b * c * gA - (a * c + b * b) * gB + 2.f * a * b * gC);
-  const float dc = idet2 * (-b * b * gA + a * b * gB - a * a * gC);
+  const G da = idet2 * (-c * c * gA + b * c * gB - b * b * gC);
+  const G db = idet2 * ((G)2. * b * c * gA - (a * c + b * b) * gB + (G)2. * a * b * gC);
+  const G dc = idet2 * (-b * b * gA + a * b * gB - a * a * gC);
   // a = U0.U0, b = U0.U1, c = U1.U1
-  const float dU00 = 2.f * da * U00 + db * U10, dU01 = 2.f * da * U01 + db * U11, dU02 = 2.f * da * U02 + db * U12;
-  const float dU10 = 2.f * dc * U10 + db * U00, dU11 = 2.f * dc * U11 + db * U01, dU12 = 2.f * dc * U12 + db * U02;
+  const G dU00 = (G)2. * da * U00 + db * U10, dU01 = (G)2. * da * U01 + db * U11, dU02 = (G)2. * da * U02 + db * U12;
+  const G dU10 = (G)2. * dc * U10 + db * U00, dU11 = (G)2. * dc * U11 + db * U01, dU12 = (G)2. * dc * U12 + db * U02;
   // U = T M:  dT = dU M^T,  dM = T^T dU
-  const float dT00 = dU00 * M00 + dU01 * M01 + dU02 * M02, dT01 = dU00 * M10 + dU01 * M11 + dU02 * M12, dT02 = dU00 * M20 + dU01 * M21 + dU02 * M22;
-  const float dT10 = dU10 * M00 + dU11 * M01 + dU12 * M02, dT11 = dU10 * M10 + dU11 * M11 + dU12 * M12, dT12 = dU10 * M20 + dU11 * M21 + dU12 * M22;
-  const float dM00 = T00 * dU00 + T10 * dU10, dM01 = T00 * dU01 + T10 * dU11, dM02 = T00 * dU02 + T10 * dU12;
-  const float dM10 = T01 * dU00 + T11 * dU10, dM11 = T01 * dU01 + T11 * dU11, dM12 = T01 * dU02 + T11 * dU12;
-  const float dM20 = T02 * dU00 + T12 * dU10, dM21 = T02 * dU01 + T12 * dU11, dM22 = T02 * dU02 + T12 * dU12;
+  const G dT00 = dU00 * M00 + dU01 * M01 + dU02 * M02, dT01 = dU00 * M10 + dU01 * M11 + dU02 * M12, dT02 = dU00 * M20 + dU01 * M21 + dU02 * M22;
+  const G dT10 = dU10 * M00 + dU11 * M01 + dU12 * M02, dT11 = dU10 * M10 + dU11 * M11 + dU12 * M12, dT12 = dU10 * M20 + dU11 * M21 + dU12 * M22;
+  const G dM00 = T00 * dU00 + T10 * dU10, dM01 = T00 * dU01 + T10 * dU11, dM02 = T00 * dU02 + T10 * dU12;
+  const G dM10 = T01 * dU00 + T11 * dU10, dM11 = T01 * dU01 + T11 * dU11, dM12 = T01 * dU02 + T11 * dU12;
+  const G dM20 = T02 * dU00 + T12 * dU10, dM21 = T02 * dU01 + T12 * dU11, dM22 = T02 * dU02 + T12 * dU12;
   // M = Rot diag(s)
-  const float ds0 = dM00 * r00 + dM10 * r10 + dM20 * r20;
-  const float ds1 = dM01 * r01 + dM11 * r11 + dM21 * r21;
-  const float ds2 = dM02 * r02 + dM12 * r12 + dM22 * r22;
-  dL_dlog_scales[3 * i] = ds0 * s0;
-  dL_dlog_scales[3 * i + 1] = ds1 * s1;
-  dL_dlog_scales[3 * i + 2] = ds2 * s2;
-  const float dr00 = dM00 * s0, dr01 = dM01 * s1, dr02 = dM02 * s2;
-  const float dr10 = dM10 * s0, dr11 = dM11 * s1, dr12 = dM12 * s2;
-  const float dr20 = dM20 * s0, dr21 = dM21 * s1, dr22 = dM22 * s2;
+  const G ds0 = dM00 * r00 + dM10 * r10 + dM20 * r20;
+  const G ds1 = dM01 * r01 + dM11 * r11 + dM21 * r21;
+  const G ds2 = dM02 * r02 + dM12 * r12 + dM22 * r22;
+  dL_dlog_scales[3 * i] = (float)(ds0 * s0);
+  dL_dlog_scales[3 * i + 1] = (float)(ds1 * s1);
+  dL_dlog_scales[3 * i + 2] = (float)(ds2 * s2);
+  const G dr00 = dM00 * s0, dr01 = dM01 * s1, dr02 = dM02 * s2;
+  const G dr10 = dM10 * s0, dr11 = dM11 * s1, dr12 = dM12 * s2;
+  const G dr20 = dM20 * s0, dr21 = dM21 * s1, dr22 = dM22 * s2;
   // Rot(unit quaternion)
-  const float dqw = 2.f * (-qz * dr01 + qy * dr02 + qz * dr10 - qx * dr12 - qy * dr20 + qx * dr21);
-  const float dqx = 2.f * (qy * dr01 + qz * dr02 + qy * dr10 - 2.f * qx * dr11 - qw * dr12 + qz * dr20 + qw * dr21 - 2.f * qx * dr22);
-  const float dqy = 2.f * (-2.f * qy * dr00 + qx * dr01 + qw * dr02 + qx * dr10 + qz * dr12 - qw * dr20 + qz * dr21 - 2.f * qy * dr22);
-  const float dqz = 2.f * (-2.f * qz * dr00 - qw * dr01 + qx * dr02 + qw * dr10 - 2.f * qz * dr11 + qy * dr12 + qx * dr20 + qy * dr21);
+  const G dqw = (G)2. * (-qz * dr01 + qy * dr02 + qz * dr10 - qx * dr12 - qy * dr20 + qx * dr21);
+  const G dqx = (G)2. * (qy * dr01 + qz * dr02 + qy * dr10 - (G)2. * qx * dr11 - qw * dr12 + qz * dr20 + qw * dr21 - (G)2. * qx * dr22);
+  const G dqy = (G)2. * (-(G)2. * qy * dr00 + qx * dr01 + qw * dr02 + qx * dr10 + qz * dr12 - qw * dr20 + qz * dr21 - (G)2. * qy * dr22);
+  const G dqz = (G)2. * (-(G)2. * qz * dr00 - qw * dr01 + qx * dr02 + qw * dr10 - (G)2. * qz * dr11 + qy * dr12 + qx * dr20 + qy * dr21);
   // through q / |q|
-  const float qdot = qw * dqw + qx * dqx + qy * dqy + qz * dqz;
-  dL_dquats[i] = make_float4((dqw - qw * qdot) * qinv, (dqx - qx * qdot) * qinv, (dqy - qy * qdot) * qinv, (dqz - qz * qdot) * qinv);
+  const G qdot = qw * dqw + qx * dqx + qy * dqy + qz * dqz;
+  dL_dquats[i] = make_float4((float)((dqw - qw * qdot) * qinv), (float)((dqx - qx * qdot) * qinv), (float)((dqy - qy * qdot) * qinv), (float)((dqz - qz * qdot) * qinv));
   // T = J W
-  const float dJ00 = dT00 * R[0] + dT01 * R[1] + dT02 * R[2];
-  const float dJ02 = dT00 * R[6] + dT01 * R[7] + dT02 * R[8];
-  const float dJ11 = dT10 * R[3] + dT11 * R[4] + dT12 * R[5];
-  const float dJ12 = dT10 * R[6] + dT11 * R[7] + dT12 * R[8];
+  const G dJ00 = dT00 * Rd[0] + dT01 * Rd[1] + dT02 * Rd[2];
+  const G dJ02 = dT00 * Rd[6] + dT01 * Rd[7] + dT02 * Rd[8];
+  const G dJ11 = dT10 * Rd[3] + dT11 * Rd[4] + dT12 * Rd[5];
+  const G dJ12 = dT10 * Rd[6] + dT11 * Rd[7] + dT12 * Rd[8];
   // J(t) and the projected centre
-  const float iz2 = iz * iz;
-  float dtx = gm.x * cam.fx * iz, dty = gm.y * cam.fy * iz;
-  float dtz = -(dJ00 * cam.fx + dJ11 * cam.fy) * iz2 - (gm.x * cam.fx * tx + gm.y * cam.fy * ty) * iz2;
-  if (xcl) dtz += dJ02 * cam.fx * xz * iz2;  // J02 = -fx L / z with L = +-limx
-  else { dtx += -dJ02 * cam.fx * iz2; dtz += dJ02 * 2.f * cam.fx * tx * iz2 * iz; }
-  if (ycl) dtz += dJ12 * cam.fy * yz * iz2;
-  else { dty += -dJ12 * cam.fy * iz2; dtz += dJ12 * 2.f * cam.fy * ty * iz2 * iz; }
+  const G iz2 = iz * iz;
+  G dtx = gm.x * fxd * iz, dty = gm.y * fyd * iz;
+  G dtz = -(dJ00 * fxd + dJ11 * fyd) * iz2 - ((G)gm.x * fxd * tx + (G)gm.y * fyd * ty) * iz2;
+  if (xcl) dtz += dJ02 * fxd * xz * iz2;  // J02 = -fx L / z with L = +-limx
+  else { dtx += -dJ02 * fxd * iz2; dtz += dJ02 * (G)2. * fxd * tx * iz2 * iz; }
+  if (ycl) dtz += dJ12 * fyd * yz * iz2;
+  else { dty += -dJ12 * fyd * iz2; dtz += dJ12 * (G)2. * fyd * ty * iz2 * iz; }
   // t = R p + t_cam
-  dmx += R[0] * dtx + R[3] * dty + R[6] * dtz;
-  dmy += R[1] * dtx + R[4] * dty + R[7] * dtz;
-  dmz += R[2] * dtx + R[5] * dty + R[8] * dtz;
-  dL_dmeans[3 * i] = dmx;
-  dL_dmeans[3 * i + 1] = dmy;
-  dL_dmeans[3 * i + 2] = dmz;
-  dL_dopacity_logits[i] = dL_dopacity[i] * o * (1.f - o);
+  const G dmx_g = Rd[0] * dtx + Rd[3] * dty + Rd[6] * dtz;
+  const G dmy_g = Rd[1] * dtx + Rd[4] * dty + Rd[7] * dtz;
+  const G dmz_g = Rd[2] * dtx + Rd[5] * dty + Rd[8] * dtz;
+  dL_dmeans[3 * i] = (float)((G)dmx + dmx_g);
+  dL_dmeans[3 * i + 1] = (float)((G)dmy + dmy_g);
+  dL_dmeans[3 * i + 2] = (float)((G)dmz + dmz_g);
+  dL_dopacity_logits[i] = dL_dopacity[i] * o * ((G)1. - o);
 }
 
 }  // namespace

@@ -113,6 +113,7 @@ __global__ void __launch_bounds__(RN_THREADS) render_bwd_kernel(
   uint32_t bmax = 0;
 #pragma unroll
   for (int w = 0; w < RN_THREADS / 32; w++) bmax = max(bmax, wmax_sh[w]);
+  bmax = min(bmax, range.y - range.x);  // never walk past the tile's own list
   if (bmax == 0) return;
 
   // where this lane's reduced sum goes

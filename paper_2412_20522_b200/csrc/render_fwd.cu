@@ -150,7 +150,7 @@ extern "C" int mg_render_fwd(const mg_camera* cam, const uint32_t* sorted_ids, c
                              float* image, float* final_T, uint32_t* n_contrib, void* stream) {
   if (int rc = mg_check_camera(cam)) return rc;
   MG_REQUIRE(tile_ranges && image && final_T && n_contrib, "null output or tile_ranges");
-  MG_REQUIRE(means2d && conic_opacity && rgb && masks, "null splat array");
+  // splat arrays are dereferenced only through non-empty tile ranges (they may be null when N = 0)
   const int gw = mg_grid_w(cam), gh = mg_grid_h(cam);
   render_fwd_kernel<<<gw * gh, RN_THREADS, 0, (cudaStream_t)stream>>>(
       cam->width, cam->height, gw, cam->bg[0], cam->bg[1], cam->bg[2], sorted_ids, (const uint2*)tile_ranges,

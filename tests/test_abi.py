@@ -1,0 +1,100 @@
+"""CPU-side checks of the boundary: libmg.so builds, loads and exports every symbol include/mg.h declares;
+argument validation that needs no GPU; the product never routes through the oracle."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2412_20522_b200 import build, binding
+
+    build.build()
+    return binding.lib()
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "mg.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(mg_[a-z_]+)\s*\(", text)))
+
+
+def test_header_declares_the_five_calls():
+    syms = declared_symbols()
+    for s in ("mg_preprocess", "mg_bin_sort", "mg_render_fwd", "mg_render_bwd", "mg_preprocess_bwd"):
+        assert s in syms
+
+
+def test_library_exports_every_declared_symbol(lib):
+    from paper_2412_20522_b200 import binding
+
+    for s in declared_symbols():
+        assert hasattr(lib, s), f"libmg.so does not export {s}"
+    assert sorted(binding.EXPORTS) == declared_symbols()
+    assert lib.mg_version() >= 100
+
+
+def test_workspace_bytes_host_logic(lib):
+    from paper_2412_20522_b200 import binding
+
+    assert binding.mg_workspace_bytes(-1, 64, 64, 10) == 0
+    assert binding.mg_workspace_bytes(10, 0, 64, 10) == 0
+    assert binding.mg_workspace_bytes(10, 64, 64, 1 << 32) == 0
+    small = binding.mg_workspace_bytes(1000, 128, 128, 3000)
+    big = binding.mg_workspace_bytes(1000, 128, 128, 3_000_000)
+    assert 0 < small < big
+    # <= 256 tiles: one tile pass, so no second ping-pong buffer (8 B per key); more tiles: 16 B per key
+    one = binding.mg_workspace_bytes(0, 256, 256, 1_000_000)
+    two = binding.mg_workspace_bytes(0, 512, 512, 1_000_000)
+    assert one < 8.5e6 and 16e6 <= two < 17e6
+
+
+def test_invalid_arguments_are_rejected_without_a_gpu(lib):
+    from paper_2412_20522_b200 import binding
+
+    cam = binding.mg_camera()
+    cam.width, cam.height, cam.fx, cam.fy, cam.sh_degree = 64, 64, 50.0, 50.0, 7
+    rc = lib.mg_render_fwd(C.byref(cam), *[C.c_void_p(0)] * 10)
+    assert rc == binding.MG_ERR_INVALID_ARG and b"sh_degree" in lib.mg_last_error_string()
+    cam.sh_degree = 0
+    rc = lib.mg_render_fwd(C.byref(cam), *[C.c_void_p(0)] * 10)
+    assert rc == binding.MG_ERR_INVALID_ARG and b"null" in lib.mg_last_error_string()
+    rc = lib.mg_bin_sort(C.byref(cam), C.c_int64(-5), *[C.c_void_p(0)] * 3, C.c_uint64(0), C.c_void_p(0), C.c_size_t(0),
+                         *[C.c_void_p(0)] * 4)
+    assert rc == binding.MG_ERR_INVALID_ARG
+    rc = lib.mg_preprocess(None, C.c_int64(1), *[C.c_void_p(0)] * 15)
+    assert rc == binding.MG_ERR_INVALID_ARG
+
+
+def test_product_never_touches_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2412_20522_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle", src, flags=re.M), f
+                assert "mg_oracle" not in src and "libmg_oracle" not in src, f
+    orc_src = open(os.path.join(ROOT, "oracle", "mg_oracle.cpp")).read() + open(os.path.join(ROOT, "oracle", "__init__.py")).read()
+    assert "paper_2412_20522_b200" not in orc_src.replace("paper_2412_20522_b200/csrc (the", "").replace("paper_2412_20522_b200 never", "")
+    assert '#include "mg' not in orc_src
+
+
+def test_constants_agree_between_header_and_oracle():
+    """The oracle keeps its own copy of the readings (no shared header); the values must coincide."""
+    h = open(os.path.join(ROOT, "include", "mg.h")).read()
+    o = open(os.path.join(ROOT, "oracle", "mg_oracle.cpp")).read()
+
+    def hv(name):
+        return re.search(rf"#define {name} (.*?)\s*/\*", h).group(1).strip()
+
+    def ov(name):
+        return re.search(rf"const (?:double|int) {name} = ([^;]+);", o).group(1).strip()
+
+    ev = lambda s: eval(s.replace("f", ""))
+    for a, b in (("MG_TILE", "TILE"), ("MG_ALPHA_MIN", "ALPHA_MIN"), ("MG_ALPHA_MAX", "ALPHA_MAX"), ("MG_T_MIN", "T_MIN"),
+                 ("MG_DILATION", "DILATION"), ("MG_ZNEAR", "ZNEAR"), ("MG_JCLAMP", "JCLAMP"), ("MG_EIG_FLOOR", "EIG_FLOOR")):
+        assert abs(ev(hv(a)) - ev(ov(b))) < 1e-12, (a, hv(a), ov(b))

@@ -1,0 +1,86 @@
+"""Parity at BASELINE.json's full size (configs[2]: 3 M Gaussians, 1297x840, SH degree 3) in the launch
+configuration bench.py times.  Projection, sort and projection-backward are compared in full; the two
+blend kernels on a seeded sample of tiles the oracle can walk in seconds (the other tiles' ranges are
+emptied for both sides, which leaves the sampled tiles' arithmetic untouched)."""
+import numpy as np
+import pytest
+import torch
+
+import parity_util as pu
+from paper_2412_20522_b200 import binding as mg
+from paper_2412_20522_b200 import scenes
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def full(oracle):
+    sc = scenes.config3()
+    fr, g, m, gimg = pu.run_gpu(sc)
+    return sc, fr, g, m, gimg
+
+
+def test_full_size_projection_and_sort(full, oracle):
+    sc, fr, *_ = full
+    cam = sc.camera
+    s1 = pu.check_preprocess(fr, sc, cam, max_flag_frac=0.02)
+    ids, ranges = pu.check_bin_sort(fr, cam)
+    assert fr.R > 10_000_000
+    print("cfg3 preprocess", s1, "R", fr.R)
+
+
+def test_full_size_blend_on_sampled_tiles(full, oracle):
+    sc, fr, g, m, gimg = full
+    cam = sc.camera
+    gw, gh = mg.grid(cam)
+    rng = np.random.default_rng(12)
+    lens = (pu.u32(fr.tile_ranges)[:, 1] - pu.u32(fr.tile_ranges)[:, 0]).astype(np.int64)
+    tiles = set(rng.choice(gw * gh, 40, replace=False).tolist())
+    tiles |= {int(np.argmax(lens)), gw - 1, gw * gh - 1, gw * (gh - 1)}  # longest list + ragged corners
+    tiles = sorted(tiles)
+    ranges_full = pu.u32(fr.tile_ranges).copy()
+    ranges_s = np.zeros_like(ranges_full)
+    ranges_s[tiles] = ranges_full[tiles]
+    ids = pu.u32(fr.sorted_ids)[: fr.R]
+    ref, s3 = pu.check_render_fwd(fr, cam, sc.masks, ids, ranges_s, tiles=tiles, max_flag_frac=0.05)
+    print("cfg3 fwd sampled tiles", len(tiles), s3)
+    # backward restricted to the same tiles on both sides
+    keep_ranges = fr.tile_ranges.clone()
+    fr.tile_ranges.copy_(torch.from_numpy(ranges_s.view(np.int32)).cuda())
+    fr.render_bwd(m, gimg)
+    torch.cuda.synchronize()
+    try:
+        _, s4 = pu.check_render_bwd(fr, cam, sc.N, sc.masks, ids, ranges_s, sc.dL_dimage(), max_flag_frac=0.3)
+        print("cfg3 bwd sampled tiles", {k: round(v, 4) for k, v in s4.items()})
+    finally:
+        fr.tile_ranges.copy_(keep_ranges)
+        fr.render_bwd(m, gimg)
+        torch.cuda.synchronize()
+
+
+def test_full_size_projection_backward(full, oracle):
+    sc, fr, *_ = full
+    cam = sc.camera
+    ref5, s5 = pu.check_preprocess_bwd(fr, sc, cam)
+    for k, v in s5.items():
+        assert v <= 2e-4, f"{k}: relative 2-norm error {v:.2e}"
+    print("cfg3 preprocess_bwd", s5)
+
+
+def test_full_size_invariants(full):
+    """Properties that hold at any size: partition of unity (Eq. 16 telescoped) and range bookkeeping."""
+    sc, fr, g, m, gimg = full
+    ranges = pu.u32(fr.tile_ranges).astype(np.int64)
+    assert (ranges[:, 1] >= ranges[:, 0]).all() and ranges[-1, 1] == fr.R and ranges[0, 0] == 0
+    assert (ranges[1:, 0] == ranges[:-1, 1]).all()
+    assert int(pu.u32(fr.tiles_touched).astype(np.int64).sum()) == fr.R
+    # white splats, black background: image + final_T == 1 at every pixel
+    rgb_keep = fr.rgb.clone()
+    fr.rgb.fill_(1.0)
+    fr.render_fwd(m)
+    torch.cuda.synchronize()
+    s = fr.image[0] + fr.final_T
+    assert float((s - 1).abs().max()) < 2e-5
+    fr.rgb.copy_(rgb_keep)
+    fr.render_fwd(m)
+    torch.cuda.synchronize()
