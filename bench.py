@@ -1,0 +1,321 @@
+#!/usr/bin/env python
+"""bench.py -- one "step" = one pass of the whole hot path (the 5 C-ABI calls of include/mg.h) over one
+synthetic frame.  Prints ONE JSON line (see the contract in DESIGN.md "Measurement").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl reference]
+
+value = Gaussian-pixel blends per second (forward + backward blends of the frame, exact counts from
+oracle/work_counts.json, divided by the device time of a whole step), inputs resident in HBM.
+e2e    = the same with host buffers: pinned-host -> device copies of every input and device -> host reads
+         of the image and all gradients inside the timed region.
+roofline = the dominant kernel (largest share of the step), FP32-ALU bound, against the FP32 peak
+         derived in DESIGN.md (148 SMs x 128 lanes x 2 flop x sm_max_mhz).
+cpu_baseline / --impl reference = the oracle, as it stands, on the host cores, on a bounded sample of tiles.
+N > 1: one process per GPU (torchrun), replicas only -- no collective on the data path.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+# algorithmic flops (counted once from the oracle's O10/O11 arithmetic)
+FLOP_PAIR = 13        # per pair evaluation: 2 sub, 6 quadratic form, mul, min, 2 compares (+1 MUFU not counted)
+FLOP_BLEND_FWD = 11   # per blend, forward
+FLOP_BLEND_BWD = 59   # per blend, backward (49 + 10 adds of the per-entry reduction)
+KERNELS_PER_STEP = {"preprocess": 1, "bin_sort_fixed": 17, "bin_sort_per_tile_pass": 3, "render_fwd": 1,
+                    "render_bwd": 1, "preprocess_bwd": 1}
+
+
+def work_counts(cfg):
+    p = os.path.join(ROOT, "oracle", "work_counts.json")
+    data = json.load(open(p)) if os.path.exists(p) else {}
+    return data.get(str(cfg))
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows = []
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-i", str(index), "-lms", "50"], stdout=subprocess.PIPE, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        self.t.join(timeout=2)
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_sample(cfg, n_tiles_target=None, seed=0):
+    """Time the oracle on a bounded sample of the workload: every k-th tile.  Returns (blends, seconds, info)."""
+    import oracle as orc
+    from paper_2412_20522_b200 import scenes
+
+    sc = scenes.make(cfg)
+    cam = sc.camera
+    gw, gh = orc.grid(cam)
+    ntiles = gw * gh
+    if n_tiles_target is None:
+        n_tiles_target = max(96, ntiles // 4)  # ~10-30 s of CPU work at config 3
+    stride = max(1, ntiles // n_tiles_target)
+    sel = np.zeros(ntiles, np.uint8)
+    sel[seed % stride::stride] = 1
+    frac = float(sel.sum()) / ntiles
+    arrs = (sc.means, sc.log_scales, sc.quats, sc.opacity_logits, sc.sh)
+    g = sc.dL_dimage().astype(np.float64)
+    t0 = time.perf_counter()
+    pre = orc.preprocess(cam, *arrs)
+    t1 = time.perf_counter()
+    ids, ranges = orc.bin_sort(cam, pre["depths"].astype(np.float32), pre["rects"], pre["tiles_touched"], sel)
+    t2 = time.perf_counter()
+    fwd = orc.render_fwd(cam, ids, ranges, pre["means2d"], pre["conic_opacity"], pre["rgb"], sc.masks)
+    t3 = time.perf_counter()
+    rb = orc.render_bwd(cam, sc.N, ids, ranges, pre["means2d"], pre["conic_opacity"], pre["rgb"], sc.masks, g)
+    t4 = time.perf_counter()
+    orc.preprocess_bwd(cam, *arrs, rb["dL_dmeans2d"], rb["dL_dconic"], rb["dL_dopacity"], rb["dL_drgb"])
+    t5 = time.perf_counter()
+    blends = fwd["blends"] + rb["blends"]
+    # per-Gaussian steps run on the whole scene; charge the sample its share of them
+    seconds = (t3 - t2) + (t4 - t3) + (t2 - t1) + frac * ((t1 - t0) + (t5 - t4))
+    info = (f"{int(sel.sum())} of {ntiles} tiles (every {stride}th) of config {cfg}: oracle bin_sort+render_fwd+render_bwd "
+            f"on those tiles ({t2 - t1:.1f}+{t3 - t2:.1f}+{t4 - t3:.1f} s) + {frac:.4f} x (preprocess {t1 - t0:.1f} s + "
+            f"preprocess_bwd {t5 - t4:.1f} s)")
+    return blends, seconds, info
+
+
+def n_threads():
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count()
+
+
+def run_reference(args, rank, world):
+    if rank != 0:
+        return
+    import oracle as orc
+
+    orc.lib()
+    for _ in range(min(args.warmup, 1)):
+        oracle_sample(args.config, n_tiles_target=16)
+    tot_b, tot_s, info = 0, 0.0, ""
+    steps = min(args.steps, 3)
+    for s in range(steps):
+        b, sec, info = oracle_sample(args.config, seed=s)
+        tot_b += b
+        tot_s += sec
+    v = tot_b / tot_s
+    line = {"impl": "reference", "metric": "gaussian_pixel_blends_per_s", "value": v, "unit": "blends/s",
+            "n_gpus": args.gpus, "steps": steps, "warmup": min(args.warmup, 1), "ms_per_step": 1e3 * tot_s / steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(args.config), "sample": info},
+            "cpu_baseline": {"value": v, "unit": "blends/s", "cores": n_threads(), "kind": "oracle", "sample": info},
+            "e2e": {"value": v, "unit": "blends/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def workload_name(cfg):
+    return {1: "configs[0] tiny: 1k Gaussians, 128x128, SH0", 2: "configs[1] small: 100k Gaussians, 512x512, SH3",
+            3: "configs[2] outdoor: 3M Gaussians, 1297x840, SH3 (north_star target)",
+            4: "configs[3] indoor: 2.8M Gaussians, 1264x832, SH3",
+            5: "configs[4] stress: 6M Gaussians, 1920x1080, SH3, camera 0"}[cfg]
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--impl", default="ours")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", 0))
+    world = int(os.environ.get("WORLD_SIZE", 1))
+    local = int(os.environ.get("LOCAL_RANK", 0))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+
+    from paper_2412_20522_b200 import binding as mg
+    from paper_2412_20522_b200 import scenes
+
+    assert torch.cuda.is_available(), "bench.py needs a GPU (no CPU fallback)"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    mg.lib()
+    args.warmup = max(args.warmup, 3)
+
+    sc = scenes.make(args.config)
+    cam = sc.camera
+    g, m = mg.upload(sc)
+    gimg_np = sc.dL_dimage()
+    gimg = torch.from_numpy(gimg_np).cuda()
+    fr = mg.Frame(cam, sc.N)
+    fr.forward(g, m)           # sizes the sort buffers from the exact R (one sync, outside the timed region)
+    fr.backward(g, m, gimg)
+    torch.cuda.synchronize()
+    R = fr.R
+    wc = work_counts(args.config)
+    if wc is not None:
+        assert wc["R"] == R or abs(wc["R"] - R) < 1e-4 * R, (wc["R"], R)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        fr.step(g, m, gimg)
+    barrier()
+    names = ["preprocess", "bin_sort", "render_fwd", "render_bwd", "preprocess_bwd"]
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(6)] for _ in range(args.steps)]
+    sampler = ClockSampler(local) if rank == 0 else None
+    barrier()
+    for s in range(args.steps):
+        e = ev[s]
+        e[0].record(); fr.preprocess(g)
+        e[1].record(); fr.bin_sort()
+        e[2].record(); fr.render_fwd(m)
+        e[3].record(); fr.render_bwd(m, gimg)
+        e[4].record(); fr.preprocess_bwd(g)
+        e[5].record()
+    barrier()
+    clocks = sampler.stop() if sampler else None
+    total_ms = ev[0][0].elapsed_time(ev[-1][5])
+    per_call = {n: float(np.mean([ev[s][i].elapsed_time(ev[s][i + 1]) for s in range(args.steps)])) for i, n in enumerate(names)}
+    assert int(fr.R_host[1]) == R
+    if world > 1:
+        t = torch.tensor([total_ms], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_step = total_ms / args.steps
+
+    # ---- e2e: host buffers, H2D of every input + D2H of image and gradients inside the timed region
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    host_in = {k: pin(getattr(sc, k)) for k in ("means", "log_scales", "quats", "opacity_logits", "sh")}
+    host_m, host_g = pin(sc.masks), pin(gimg_np)
+    out_names = ["image", "dL_dmask", "dL_dmeans", "dL_dlog_scales", "dL_dquats", "dL_dopacity_logits", "dL_dsh"]
+    host_out = {k: torch.empty(getattr(fr, k).shape, dtype=torch.float32).pin_memory() for k in out_names}
+    h2d = sum(t.numel() * 4 for t in host_in.values()) + host_m.numel() * 4 + host_g.numel() * 4
+    d2h = sum(t.numel() * 4 for t in host_out.values())
+
+    def e2e_step():
+        for k, t in host_in.items():
+            g[k].copy_(t, non_blocking=True)
+        m.copy_(host_m, non_blocking=True)
+        gimg.copy_(host_g, non_blocking=True)
+        fr.step(g, m, gimg)
+        for k, t in host_out.items():
+            t.copy_(getattr(fr, k), non_blocking=True)
+
+    e2e_step()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.e2e_steps):
+        e2e_step()
+    e1.record()
+    barrier()
+    e2e_ms = e0.elapsed_time(e1) / args.e2e_steps
+    if world > 1:
+        t = torch.tensor([e2e_ms], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    blends = (wc["fwd_blends"] + wc["bwd_blends"]) if wc else None
+    value = world * blends / (ms_step * 1e-3) if blends else None
+    e2e_value = world * blends / (e2e_ms * 1e-3) if blends else None
+
+    # ---- roofline of the dominant kernel
+    dom = max(("render_fwd", "render_bwd"), key=lambda n: per_call[n])
+    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    sm_max = 1965.0
+    if os.path.exists(peaks_path):
+        sm_max = float(json.load(open(peaks_path)).get("sm_max_mhz", sm_max))
+    fp32_peak = 148 * 128 * 2 * sm_max * 1e6 / 1e12  # TFLOP/s (derived, MEASURED_PEAKS has no FP32 entry)
+    roofline = None
+    if wc:
+        if dom == "render_bwd":
+            flops = wc["bwd_pair_evals"] * FLOP_PAIR + wc["bwd_blends"] * FLOP_BLEND_BWD
+        else:
+            flops = wc["fwd_pair_evals"] * FLOP_PAIR + wc["fwd_blends"] * FLOP_BLEND_FWD
+        ach = flops / (per_call[dom] * 1e-3) / 1e12
+        roofline = {"kernel": dom + "_kernel", "bound": "alu", "achieved": ach, "peak": fp32_peak, "unit": "TFLOP/s",
+                    "frac": ach / fp32_peak, "traffic": None, "share_of_step": per_call[dom] / sum(per_call.values()),
+                    "peak_source": f"derived 148 SM x 128 lanes x 2 x {sm_max:.0f} MHz (no FP32 entry in MEASURED_PEAKS.json)"}
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        b, sec, info = oracle_sample(args.config)
+        cpu = {"value": b / sec, "unit": "blends/s", "cores": n_threads(), "kind": "oracle", "sample": info}
+
+    gw, gh = mg.grid(cam)
+    tile_passes = 1 if gw * gh <= 256 else (2 if gw * gh <= 65536 else 3)
+    launches = args.steps * (1 + KERNELS_PER_STEP["bin_sort_fixed"] + 3 * tile_passes + 1 + 1 + 1)
+    line = {"metric": "gaussian_pixel_blends_per_s", "value": value, "unit": "blends/s", "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": workload_name(args.config), "N": sc.N, "width": cam.width, "height": cam.height,
+                       "sh_degree": cam.sh_degree, "R": R, "l2": "inputs (708 MB of Gaussians + sort buffers) exceed the 126 MB L2; no flush",
+                       "parallelism": "replicas only" if world > 1 else "1 GPU"},
+            "ms_per_frame": ms_step, "ms_per_call": per_call,
+            "pair_evals_per_s": (world * (wc["fwd_pair_evals"] + wc["bwd_pair_evals"]) / (ms_step * 1e-3)) if wc else None,
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": "blends/s", "ms_per_step": e2e_ms, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+            "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

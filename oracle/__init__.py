@@ -79,8 +79,8 @@ def preprocess(cam, means, log_scales, quats, opacity_logits, sh):
     return out
 
 
-def bin_sort(cam, depths, rects, tiles_touched):
-    """O9.  depths are taken as fp32 (their bit pattern is the sort key)."""
+def bin_sort(cam, depths, rects, tiles_touched, tile_select=None):
+    """O9.  depths are taken as fp32 (their bit pattern is the sort key).  tile_select: optional uint8 per tile."""
     N = depths.shape[0]
     depths, rects, tiles_touched = _in(depths, np.float32), _in(rects, np.int32), _in(tiles_touched, np.uint32)
     R = int(tiles_touched.astype(np.uint64).sum())
@@ -89,10 +89,12 @@ def bin_sort(cam, depths, rects, tiles_touched):
     tile_ranges = np.zeros((gw * gh, 2), np.uint32)
     R_out = C.c_uint64(0)
     c = _cam(cam)
+    sel = None if tile_select is None else _in(tile_select, np.uint8)
+    assert sel is None or sel.shape == (gw * gh,)
     rc = lib().orc_bin_sort(C.byref(c), C.c_int64(N), _p(depths), _p(rects), _p(tiles_touched), _p(sorted_ids),
-                            _p(tile_ranges), C.byref(R_out))
-    assert rc == 0 and R_out.value == R
-    return sorted_ids[:R], tile_ranges
+                            _p(tile_ranges), C.byref(R_out), None if sel is None else _p(sel))
+    assert rc == 0 and (R_out.value == R if sel is None else R_out.value <= R)
+    return sorted_ids[:R_out.value], tile_ranges
 
 
 def render_fwd(cam, sorted_ids, tile_ranges, means2d, conic_opacity, rgb, masks):

@@ -265,8 +265,10 @@ int orc_preprocess(const Cam* cam, int64_t N, const double* means, const double*
 // O9.  Global order = surviving Gaussians ascending by the fp32 bit pattern of depth, ties by
 // index (stable sort).  List of tile t = the sub-sequence of that order whose rect contains t.
 // sorted_ids must hold R = sum(tiles_touched) entries; returns R through R_out.
+// tile_select (optional, one byte per tile): tiles with a zero byte are left with an empty range, so
+// that a bounded sample of a large workload can be listed (bench.py's cpu_baseline leg).
 int orc_bin_sort(const Cam* cam, int64_t N, const float* depths, const int32_t* rects, const uint32_t* tiles_touched,
-                 uint32_t* sorted_ids, uint32_t* tile_ranges, uint64_t* R_out) {
+                 uint32_t* sorted_ids, uint32_t* tile_ranges, uint64_t* R_out, const uint8_t* tile_select) {
   const int gw = (cam->width + TILE - 1) / TILE, gh = (cam->height + TILE - 1) / TILE;
   std::vector<uint32_t> order;
   for (int64_t i = 0; i < N; i++)
@@ -278,6 +280,7 @@ int orc_bin_sort(const Cam* cam, int64_t N, const float* depths, const int32_t* 
   for (int t = 0; t < ntiles; t++) {
     const int tx = t % gw, ty = t / gw;
     uint64_t c = 0;
+    if (tile_select && !tile_select[t]) { count[t + 1] = 0; continue; }
     for (uint32_t id : order) {
       const int32_t* r = rects + 4 * (int64_t)id;
       if (tx >= r[0] && tx < r[2] && ty >= r[1] && ty < r[3]) c++;
@@ -289,6 +292,7 @@ int orc_bin_sort(const Cam* cam, int64_t N, const float* depths, const int32_t* 
   for (int t = 0; t < ntiles; t++) {
     const int tx = t % gw, ty = t / gw;
     uint64_t k = count[t];
+    if (!(tile_select && !tile_select[t]))
     for (uint32_t id : order) {
       const int32_t* r = rects + 4 * (int64_t)id;
       if (tx >= r[0] && tx < r[2] && ty >= r[1] && ty < r[3]) sorted_ids[k++] = id;
