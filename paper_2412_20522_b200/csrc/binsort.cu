@@ -1,51 +1,69 @@
-// binsort.cu -- mg_bin_sort: key duplication, (tile, depth) radix sort, tile ranges.
+// binsort.cu -- mg_bin_sort: key duplication, (tile, depth) sort, tile ranges.
 // Steps a4-a6 of the hot path (PAPER.md:66 "depth order", :74 16x16 tiles; O9).
 //
-// The result is the ascending order of the 64-bit keys (tile_id << 32 | depth bits), ties by index.
-// It is produced by an LSD radix sort of that key whose four depth-digit passes are HOISTED BEFORE
-// the key duplication: all duplicates of a Gaussian share its depth, so sorting the N Gaussians by
-// depth first (stable, 4 x 8 bits) and emitting the duplicates in that order leaves only the
-// ceil(log2(tiles)) tile bits to sort over the R duplicated keys (2 stable passes for <= 65536
-// tiles).  Per duplicated key this moves ~44 B instead of ~150 B for six 64-bit key-value passes.
-// Tile ranges come from a summed-area table of the tile rectangles (4 atomics per Gaussian), not
-// from a pass over the sorted keys.
+// The result is DEFINED as the ascending order of the 64-bit keys (tile_id << 32 | depth bits), ties
+// by Gaussian index, tile_id = ty * gw + tx.  It is produced without ever materialising those keys:
+//
+//  S1  depth order of the N Gaussians: stable LSD radix sort of the fp32 depth bits (4 x 8 bits).
+//      All duplicates of a Gaussian share its depth, so the depth digits are sorted BEFORE the
+//      duplication (N keys instead of R).
+//  S2  row expansion: Gaussian k of the depth order covers tile rows [y0, y1); it emits one record
+//      (id, x0, x1) into the list of each of those rows, lists kept in depth order.  All duplicates
+//      of a Gaussian within a tile row share (depth, ty), so the row digit is "sorted" before the
+//      expansion in x (sum(y1 - y0) records instead of R).
+//  S3  column expansion: within a row, record j covers tile columns [x0, x1); it emits its id into
+//      the list of each of those tiles, lists kept in record order.  The concatenation of the tile
+//      lists over (ty, tx) ascending is sorted_ids; the list boundaries are tile_ranges.
+//
+// S2 and S3 are the same primitive, a STABLE INTERVAL EXPANSION: items in sequence order, each with
+// an interval of bins, are appended to every bin of their interval, order preserved.  A warp takes
+// a chunk of 512 consecutive items, 32 at a time: lane k turns its interval into a row of a 32 x
+// 32-bin bit matrix, a 5-stage shuffle butterfly transposes it, and lane c then holds the set of
+// items that cover bin c, in item order.  Counting is a popc; emitting walks the set bits.  Per
+// chunk and bin the counts go to a table, an exclusive scan of the table (bin-major, chunk-minor)
+// gives every (bin, chunk) its write position, and a second sweep emits.
+//
+// Bytes moved per duplicated key: ~4 B written + ~16 B of records and tables (mostly L2 hits),
+// against ~150 B for six 64-bit key-value radix passes over R keys.
 #include "mg_common.cuh"
 
 namespace {
 
+// ---------------------------------------------------------------- S1: radix sort of the N depth keys
 constexpr int RS_THREADS = 512;
 constexpr int RS_ITEMS = 16;
 constexpr int RS_WARPS = RS_THREADS / 32;
 constexpr int RS_TILE = RS_THREADS * RS_ITEMS;  // 8192 elements per block
-constexpr int RS_MAX_BINS = 256;
+constexpr int RS_BINS = 256;
 
-struct SortCtl {           // lives in the workspace
-  unsigned long long R;    // true number of duplicated keys
-  uint32_t overflow;       // 1 if R > capacity or R >= 2^32
-  uint32_t pad;
+constexpr int XP_CHUNK = 512;   // items per warp in the expansion sweeps
+constexpr int XP_MAX_WARPS = 8; // warps per block in the expansion sweeps
+constexpr int SCAN_THREADS = 1024;
+constexpr int SCAN_ITEMS = 4;
+constexpr int SCAN_BLK = SCAN_THREADS * SCAN_ITEMS;
+
+struct SortCtl {            // lives in the workspace; zeroed at the start of every call
+  unsigned long long R;     // true number of duplicated keys = sum of tiles_touched
+  uint32_t nvis;            // Gaussians with tiles_touched > 0
+  uint32_t overflow;        // 1 if R > capacity or R >= 2^32
+  uint32_t n_chunks_c;      // chunks of the column expansion (sum over rows of ceil(records / XP_CHUNK))
+  uint32_t n_table_c;       // gw * n_chunks_c
+  uint32_t pad[2];
 };
 
-// One stable radix pass on `bits` bits at `shift`.  kCount: write the per-block digit histogram to
+// One stable radix pass on 8 bits at `shift`.  kCount: write the per-block digit histogram to
 // table[digit][block].  Otherwise: table holds the exclusive scan (digit-major) and the block
 // scatters its elements, keeping their order within a digit.
-template <bool kCount, bool kWriteKeys>
+template <bool kCount>
 __global__ void __launch_bounds__(RS_THREADS) radix_pass_kernel(
     const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in, uint32_t* __restrict__ keys_out,
-    uint32_t* __restrict__ vals_out, uint32_t n_static, const SortCtl* __restrict__ ctl, int shift, int bits,
-    uint32_t* __restrict__ table, int nblocks) {
-  __shared__ uint32_t cnt[RS_WARPS][RS_MAX_BINS];
-  __shared__ uint32_t gbase[RS_MAX_BINS];
-  const int bins = 1 << bits;
-  uint32_t n = n_static;
-  if (ctl) {
-    if (ctl->overflow) n = 0;
-    else n = (uint32_t)min((unsigned long long)n_static, ctl->R);
-  }
+    uint32_t* __restrict__ vals_out, uint32_t n, int shift, uint32_t* __restrict__ table, int nblocks) {
+  __shared__ uint32_t cnt[RS_WARPS][RS_BINS];
+  __shared__ uint32_t gbase[RS_BINS];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  for (int i = threadIdx.x; i < RS_WARPS * RS_MAX_BINS; i += RS_THREADS) (&cnt[0][0])[i] = 0;
+  for (int i = threadIdx.x; i < RS_WARPS * RS_BINS; i += RS_THREADS) (&cnt[0][0])[i] = 0;
   __syncthreads();
   const uint32_t base = blockIdx.x * (uint32_t)RS_TILE + warp * (32 * RS_ITEMS);
-  const uint32_t mask = (uint32_t)bins - 1;
   uint32_t key[RS_ITEMS], rank[RS_ITEMS];
 #pragma unroll
   for (int it = 0; it < RS_ITEMS; it++) {
@@ -56,7 +74,7 @@ __global__ void __launch_bounds__(RS_THREADS) radix_pass_kernel(
   for (int it = 0; it < RS_ITEMS; it++) {
     const uint32_t idx = base + it * 32 + lane;
     const bool valid = idx < n;
-    const uint32_t d = valid ? ((key[it] >> shift) & mask) : (uint32_t)bins;  // invalid lanes match only each other
+    const uint32_t d = valid ? ((key[it] >> shift) & 255u) : 256u;  // invalid lanes match only each other
     const uint32_t peers = __match_any_sync(0xffffffffu, d);
     uint32_t before = 0;
     if (valid) before = cnt[warp][d];
@@ -66,7 +84,7 @@ __global__ void __launch_bounds__(RS_THREADS) radix_pass_kernel(
     rank[it] = before + __popc(peers & ((1u << lane) - 1u));
   }
   __syncthreads();
-  if (threadIdx.x < bins) {
+  if (threadIdx.x < RS_BINS) {
     uint32_t s = 0;
 #pragma unroll
     for (int w = 0; w < RS_WARPS; w++) {
@@ -83,187 +101,246 @@ __global__ void __launch_bounds__(RS_THREADS) radix_pass_kernel(
   for (int it = 0; it < RS_ITEMS; it++) {
     const uint32_t idx = base + it * 32 + lane;
     if (idx < n) {
-      const uint32_t d = (key[it] >> shift) & mask;
+      const uint32_t d = (key[it] >> shift) & 255u;
       const uint32_t dst = gbase[d] + cnt[warp][d] + rank[it];
-      if (kWriteKeys) keys_out[dst] = key[it];
-      vals_out[dst] = vals_in[idx];
+      keys_out[dst] = key[it];
+      vals_out[dst] = vals_in ? vals_in[idx] : idx;  // first pass: the value is the index itself
     }
-  }
-}
-
-// In-place exclusive scan of `total` uint32 values by one block (digit-major histogram table).
-__global__ void __launch_bounds__(1024) table_scan_kernel(uint32_t* __restrict__ table, size_t total) {
-  __shared__ uint32_t part[1024];
-  const size_t chunk = (total + 1023) / 1024;
-  const size_t b = (size_t)threadIdx.x * chunk, e = min(total, b + chunk);
-  uint32_t s = 0;
-  for (size_t i = b; i < e; i++) s += table[i];
-  part[threadIdx.x] = s;
-  __syncthreads();
-  for (int o = 1; o < 1024; o <<= 1) {  // Hillis-Steele inclusive scan
-    const uint32_t v = threadIdx.x >= o ? part[threadIdx.x - o] : 0;
-    __syncthreads();
-    part[threadIdx.x] += v;
-    __syncthreads();
-  }
-  uint32_t run = part[threadIdx.x] - s;
-  for (size_t i = b; i < e; i++) {
-    const uint32_t v = table[i];
-    table[i] = run;
-    run += v;
   }
 }
 
 // Depth keys: fp32 bits of depth (positive floats order as unsigned ints); culled Gaussians last.
-__global__ void depth_keys_kernel(int64_t N, const float* __restrict__ depths, const uint32_t* __restrict__ tiles_touched,
-                                  uint32_t* __restrict__ keys, uint32_t* __restrict__ vals) {
+// Also R = sum of tiles_touched and the number of visible Gaussians.
+__global__ void __launch_bounds__(256) depth_keys_kernel(int64_t N, const float* __restrict__ depths,
+                                                         const uint32_t* __restrict__ tiles_touched,
+                                                         uint32_t* __restrict__ keys, SortCtl* __restrict__ ctl) {
+  __shared__ unsigned long long s_sum[8];
+  __shared__ uint32_t s_vis[8];
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= N) return;
-  keys[i] = tiles_touched[i] ? __float_as_uint(depths[i]) : 0xffffffffu;
-  vals[i] = (uint32_t)i;
+  uint32_t tt = 0;
+  if (i < N) {
+    tt = tiles_touched[i];
+    keys[i] = tt ? __float_as_uint(depths[i]) : 0xffffffffu;
+  }
+  const uint32_t vis = __popc(__ballot_sync(0xffffffffu, tt != 0));
+  unsigned long long sum = tt;
+#pragma unroll
+  for (int o = 16; o >= 1; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (lane == 0) { s_sum[warp] = sum; s_vis[warp] = vis; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    unsigned long long t = 0;
+    uint32_t v = 0;
+#pragma unroll
+    for (int w = 0; w < 8; w++) { t += s_sum[w]; v += s_vis[w]; }
+    if (t) atomicAdd(&ctl->R, t);
+    if (v) atomicAdd(&ctl->nvis, v);
+  }
 }
 
-__device__ __forceinline__ unsigned long long block_exclusive_scan_256(unsigned long long v, unsigned long long* total) {
-  __shared__ unsigned long long wsum[8];
+__global__ void ctl_finalize_kernel(SortCtl* __restrict__ ctl, unsigned long long capacity) {
+  ctl->overflow = (ctl->R > capacity || ctl->R >= (1ull << 32)) ? 1u : 0u;
+}
+
+// ---------------------------------------------------------------- exclusive scan of a uint32 table
+// Two launches: per-block sums, then each block adds the sums of the blocks before it and scans its
+// own part in place.  n comes from device memory when n_dev != nullptr (else n_static).  The grand
+// total is written to table[n].
+__device__ __forceinline__ uint32_t scan_n(uint32_t n_static, const uint32_t* n_dev) { return n_dev ? *n_dev : n_static; }
+
+__device__ __forceinline__ uint32_t block_reduce_1024(uint32_t v, uint32_t* sh) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  unsigned long long inc = v;
+  v = __reduce_add_sync(0xffffffffu, v);
+  __syncthreads();  // sh may still be read from a previous use
+  if (lane == 0) sh[warp] = v;
+  __syncthreads();
+  uint32_t t = sh[lane];
+  t = __reduce_add_sync(0xffffffffu, t);
+  return t;
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS) scan_sums_kernel(const uint32_t* __restrict__ table, uint32_t n_static,
+                                                                 const uint32_t* __restrict__ n_dev,
+                                                                 uint32_t* __restrict__ sums) {
+  __shared__ uint32_t sh[32];
+  const uint32_t n = scan_n(n_static, n_dev);
+  const uint32_t b0 = blockIdx.x * (uint32_t)SCAN_BLK;
+  if (b0 >= n) return;
+  uint32_t s = 0;
+#pragma unroll
+  for (int i = 0; i < SCAN_ITEMS; i++) {
+    const uint32_t idx = b0 + i * SCAN_THREADS + threadIdx.x;
+    if (idx < n) s += table[idx];
+  }
+  s = block_reduce_1024(s, sh);
+  if (threadIdx.x == 0) sums[blockIdx.x] = s;
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS) scan_apply_kernel(uint32_t* __restrict__ table, uint32_t n_static,
+                                                                  const uint32_t* __restrict__ n_dev,
+                                                                  const uint32_t* __restrict__ sums) {
+  __shared__ uint32_t sh[32];
+  __shared__ uint32_t wsum[32];
+  const uint32_t n = scan_n(n_static, n_dev);
+  const uint32_t b0 = blockIdx.x * (uint32_t)SCAN_BLK;
+  if (n == 0) {
+    if (blockIdx.x == 0 && threadIdx.x == 0) table[0] = 0;
+    return;
+  }
+  if (b0 >= n) return;
+  uint32_t pre = 0;
+  for (uint32_t j = threadIdx.x; j < blockIdx.x; j += SCAN_THREADS) pre += sums[j];
+  pre = block_reduce_1024(pre, sh);
+  // each thread owns SCAN_ITEMS consecutive elements
+  const uint32_t t0 = b0 + threadIdx.x * SCAN_ITEMS;
+  uint32_t v[SCAN_ITEMS], s = 0;
+#pragma unroll
+  for (int i = 0; i < SCAN_ITEMS; i++) {
+    v[i] = (t0 + i < n) ? table[t0 + i] : 0u;
+    s += v[i];
+  }
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  uint32_t inc = s;
 #pragma unroll
   for (int o = 1; o < 32; o <<= 1) {
-    const unsigned long long t = __shfl_up_sync(0xffffffffu, inc, o);
+    const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
     if (lane >= o) inc += t;
   }
   if (lane == 31) wsum[warp] = inc;
   __syncthreads();
-  unsigned long long woff = 0, tot = 0;
+  uint32_t woff = 0, tot = 0;
+  {
+    const uint32_t w = wsum[lane];
+    uint32_t winc = w;
 #pragma unroll
-  for (int w = 0; w < 8; w++) {
-    if (w < warp) woff += wsum[w];
-    tot += wsum[w];
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t t = __shfl_up_sync(0xffffffffu, winc, o);
+      if (lane >= o) winc += t;
+    }
+    woff = __shfl_sync(0xffffffffu, winc - w, warp);
+    tot = __shfl_sync(0xffffffffu, winc, 31);
   }
-  *total = tot;
-  return woff + inc - v;
+  uint32_t run = pre + woff + inc - s;
+#pragma unroll
+  for (int i = 0; i < SCAN_ITEMS; i++) {
+    if (t0 + i < n) table[t0 + i] = run;
+    run += v[i];
+  }
+  if (b0 + SCAN_BLK >= n && threadIdx.x == 0) table[n] = pre + tot;
 }
 
-// Block sums of tiles_touched taken in depth order.
-__global__ void __launch_bounds__(256) tt_block_sums_kernel(int64_t N, const uint32_t* __restrict__ order,
-                                                            const uint32_t* __restrict__ tiles_touched,
-                                                            unsigned long long* __restrict__ block_sums) {
-  const int64_t k = (int64_t)blockIdx.x * 256 + threadIdx.x;
-  const unsigned long long v = k < N ? tiles_touched[order[k]] : 0;
-  unsigned long long tot;
-  block_exclusive_scan_256(v, &tot);
-  if (threadIdx.x == 0) block_sums[blockIdx.x] = tot;
+// ---------------------------------------------------------------- stable interval expansion
+// Bits [lo, hi) of the 32-bin word w.
+__device__ __forceinline__ uint32_t interval_bits(int lo, int hi, int w) {
+  const int l = max(lo - 32 * w, 0), h = min(hi - 32 * w, 32);
+  if (h <= l) return 0u;
+  const uint32_t upto_h = h >= 32 ? 0xffffffffu : ((1u << h) - 1u);
+  return upto_h & ~((1u << l) - 1u);
 }
 
-// Exclusive scan of the block sums by one block; publishes R and the overflow flag.
-__global__ void __launch_bounds__(1024) block_sums_scan_kernel(unsigned long long* __restrict__ block_sums, int nblk,
-                                                               unsigned long long capacity, SortCtl* __restrict__ ctl,
-                                                               int32_t* __restrict__ sat, int sat_n) {
-  __shared__ unsigned long long part[1024];
-  const int chunk = (nblk + 1023) / 1024;
-  const int b = threadIdx.x * chunk, e = min(nblk, b + chunk);
-  unsigned long long s = 0;
-  for (int i = b; i < e; i++) s += block_sums[i];
-  part[threadIdx.x] = s;
-  __syncthreads();
-  for (int o = 1; o < 1024; o <<= 1) {
-    const unsigned long long v = threadIdx.x >= o ? part[threadIdx.x - o] : 0;
-    __syncthreads();
-    part[threadIdx.x] += v;
-    __syncthreads();
+// 32 x 32 bit-matrix transpose across a warp: in, lane k holds row k (bit c = column c); out, lane c
+// holds column c (bit k = row k).
+__device__ __forceinline__ uint32_t transpose32(uint32_t x, int lane) {
+#pragma unroll
+  for (int j = 16; j >= 1; j >>= 1) {
+    const uint32_t m = j == 16 ? 0x0000ffffu : j == 8 ? 0x00ff00ffu : j == 4 ? 0x0f0f0f0fu : j == 2 ? 0x33333333u : 0x55555555u;
+    const uint32_t y = __shfl_xor_sync(0xffffffffu, x, j);
+    if (lane & j) x = ((y >> j) & m) | (x & ~m);
+    else x = (x & m) | ((y << j) & ~m);
   }
-  unsigned long long run = part[threadIdx.x] - s;
-  for (int i = b; i < e; i++) {
-    const unsigned long long v = block_sums[i];
-    block_sums[i] = run;
-    run += v;
-  }
-  if (threadIdx.x == 1023) {
-    ctl->R = part[1023];
-    ctl->overflow = (part[1023] > capacity || part[1023] >= (1ull << 32)) ? 1u : 0u;
-  }
-  for (int i = threadIdx.x; i < sat_n; i += 1024) sat[i] = 0;
+  return x;
 }
 
-// Key duplication in depth order: entry k of the depth order writes its tile ids (row-major over its
-// rectangle) at offset[k].  Rectangles with more than 16 tiles are written by the whole warp.
-// Also scatters the four corners of the rectangle into the summed-area table.
-__global__ void __launch_bounds__(256) duplicate_kernel(int64_t N, const uint32_t* __restrict__ order,
-                                                        const uint32_t* __restrict__ tiles_touched,
-                                                        const int4* __restrict__ rects,
-                                                        const unsigned long long* __restrict__ block_offsets,
-                                                        const SortCtl* __restrict__ ctl, int gw, int gh,
-                                                        uint32_t* __restrict__ tile_keys, uint32_t* __restrict__ ids,
-                                                        int32_t* __restrict__ sat) {
-  if (ctl->overflow) return;
-  const int64_t k = (int64_t)blockIdx.x * 256 + threadIdx.x;
-  uint32_t id = 0, cnt = 0;
-  int4 r = make_int4(0, 0, 0, 0);
-  if (k < N) {
-    id = order[k];
-    cnt = tiles_touched[id];
-    if (cnt) r = rects[id];
-  }
-  unsigned long long tot;
-  const unsigned long long off64 = block_offsets[blockIdx.x] + block_exclusive_scan_256(cnt, &tot);
-  const uint32_t off = (uint32_t)off64;
-  if (cnt) {
-    const int sw = gw + 1;
-    atomicAdd(&sat[r.y * sw + r.x], 1);
-    atomicAdd(&sat[r.y * sw + r.z], -1);
-    atomicAdd(&sat[r.w * sw + r.x], -1);
-    atomicAdd(&sat[r.w * sw + r.z], 1);
-  }
-  const int lane = threadIdx.x & 31;
-  const bool big = cnt > 16;
-  if (cnt && !big) {
-    uint32_t o = off;
-    for (int y = r.y; y < r.w; y++)
-      for (int x = r.x; x < r.z; x++) {
-        tile_keys[o] = (uint32_t)(y * gw + x);
-        ids[o] = id;
-        o++;
+// Word range [wlo, whi] touched by the valid intervals of a warp's 32 items (whi < wlo if none).
+__device__ __forceinline__ void word_range(int lo, int hi, int* wlo, int* whi) {
+  const bool any = hi > lo;
+  *wlo = (int)__reduce_min_sync(0xffffffffu, any ? (uint32_t)(lo >> 5) : 0x7fffffffu);
+  *whi = (int)__reduce_max_sync(0xffffffffu, any ? (hi - 1) >> 5 : -1);
+}
+
+// S2: row expansion.  Item k of the depth order (k < nvis) covers rows [y0, y1).
+// kCount: table_r[row * n_chunks + chunk] = number of records of this chunk in that row; also stores the
+// packed rectangle in depth order for the second sweep.  Otherwise table_r is scanned and the records
+// (id, x0 | x1 << 16) are written to row_rec at their positions.
+template <bool kCount>
+__global__ void __launch_bounds__(32 * XP_MAX_WARPS) row_expand_kernel(
+    const uint32_t* __restrict__ order, const int4* __restrict__ rects, const SortCtl* __restrict__ ctl, int gh,
+    uint32_t n_chunks, int warps_per_block, uint2* __restrict__ prect, uint32_t* __restrict__ table_r,
+    uint2* __restrict__ row_rec) {
+  extern __shared__ uint32_t xp_smem[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t chunk = blockIdx.x * (uint32_t)warps_per_block + warp;
+  if (chunk >= n_chunks) return;
+  if (!kCount && ctl->overflow) return;
+  uint32_t* cnt = xp_smem + (size_t)warp * gh;
+  const uint32_t nvis = ctl->nvis;
+  const uint32_t k0 = chunk * (uint32_t)XP_CHUNK;
+  for (int b = lane; b < gh; b += 32) cnt[b] = kCount ? 0u : table_r[(size_t)b * n_chunks + chunk];
+  __syncwarp();
+  if (k0 < nvis) {
+    const uint32_t k1 = min(k0 + (uint32_t)XP_CHUNK, nvis);
+    for (uint32_t kb = k0; kb < k1; kb += 32) {
+      const uint32_t k = kb + lane;
+      uint32_t id = 0, xx = 0;
+      int lo = 0, hi = 0;
+      if (k < k1) {
+        id = order[k];
+        if (kCount) {
+          const int4 r = rects[id];
+          xx = (uint32_t)r.x | ((uint32_t)r.z << 16);
+          lo = r.y; hi = r.w;
+          prect[k] = make_uint2(xx, (uint32_t)r.y | ((uint32_t)r.w << 16));
+        } else {
+          const uint2 p = prect[k];
+          xx = p.x;
+          lo = (int)(p.y & 0xffffu); hi = (int)(p.y >> 16);
+        }
       }
-  }
-  uint32_t todo = __ballot_sync(0xffffffffu, big);
-  while (todo) {
-    const int src = __ffs(todo) - 1;
-    todo &= todo - 1;
-    const uint32_t bid = __shfl_sync(0xffffffffu, id, src), bcnt = __shfl_sync(0xffffffffu, cnt, src);
-    const uint32_t boff = __shfl_sync(0xffffffffu, off, src);
-    const int bx0 = __shfl_sync(0xffffffffu, r.x, src), by0 = __shfl_sync(0xffffffffu, r.y, src);
-    const int bw = __shfl_sync(0xffffffffu, r.z, src) - bx0;
-    for (uint32_t j = lane; j < bcnt; j += 32) {
-      const int y = by0 + (int)(j / (uint32_t)bw), x = bx0 + (int)(j % (uint32_t)bw);
-      tile_keys[boff + j] = (uint32_t)(y * gw + x);
-      ids[boff + j] = bid;
+      int wlo, whi;
+      word_range(lo, hi, &wlo, &whi);
+      for (int w = wlo; w <= whi; w++) {
+        uint32_t col = transpose32(interval_bits(lo, hi, w), lane);
+        const int bin = 32 * w + lane;
+        if (kCount) {
+          if (col) cnt[bin] += __popc(col);  // col != 0 implies bin < gh
+        } else {
+          uint32_t p = col ? cnt[bin] : 0u;
+          const bool mine = col != 0;
+          while (__any_sync(0xffffffffu, col != 0)) {
+            const int src = col ? __ffs(col) - 1 : 0;
+            const uint32_t vid = __shfl_sync(0xffffffffu, id, src);
+            const uint32_t vxx = __shfl_sync(0xffffffffu, xx, src);
+            if (col) {
+              row_rec[p++] = make_uint2(vid, vxx);
+              col &= col - 1;
+            }
+          }
+          if (mine) cnt[bin] = p;
+        }
+      }
     }
   }
+  if (kCount) {
+    __syncwarp();
+    for (int b = lane; b < gh; b += 32) table_r[(size_t)b * n_chunks + chunk] = cnt[b];
+  }
 }
 
-// Tile ranges from the summed-area table: 2D prefix sum -> keys per tile -> exclusive scan.
-__global__ void __launch_bounds__(1024) tile_ranges_kernel(int32_t* __restrict__ sat, int gw, int gh,
-                                                           const SortCtl* __restrict__ ctl, uint32_t* __restrict__ tile_ranges) {
+// Plan of the column expansion: records per row -> chunks per row -> chunk_base (exclusive scan over
+// rows).  One block.  row_start[r] = position of row r's first record in row_rec (r = 0..gh).
+__global__ void __launch_bounds__(1024) plan_kernel(const uint32_t* __restrict__ table_r, uint32_t n_chunks_r, int gh,
+                                                    int gw, uint32_t* __restrict__ row_start,
+                                                    uint32_t* __restrict__ chunk_base, SortCtl* __restrict__ ctl) {
   __shared__ uint32_t part[1024];
-  const int ntiles = gw * gh, sw = gw + 1;
-  if (ctl->overflow) {
-    for (int t = threadIdx.x; t < ntiles; t += 1024) { tile_ranges[2 * t] = 0; tile_ranges[2 * t + 1] = 0; }
-    return;
-  }
-  for (int y = threadIdx.x; y < gh; y += 1024) {  // prefix along x
-    int run = 0;
-    for (int x = 0; x < gw; x++) { run += sat[y * sw + x]; sat[y * sw + x] = run; }
-  }
-  __syncthreads();
-  for (int x = threadIdx.x; x < gw; x += 1024) {  // prefix along y: sat[y][x] = keys of tile (x, y)
-    int run = 0;
-    for (int y = 0; y < gh; y++) { run += sat[y * sw + x]; sat[y * sw + x] = run; }
-  }
-  __syncthreads();
-  const int chunk = (ntiles + 1023) / 1024;
-  const int b = threadIdx.x * chunk, e = min(ntiles, b + chunk);
+  const int per = (gh + 1023) / 1024;
+  const int b = threadIdx.x * per, e = min(gh, b + per);
   uint32_t s = 0;
-  for (int t = b; t < e; t++) s += (uint32_t)sat[(t / gw) * sw + (t % gw)];
+  for (int r = b; r < e; r++) {
+    const uint32_t st = table_r[(size_t)r * n_chunks_r], en = table_r[(size_t)(r + 1) * n_chunks_r];
+    row_start[r] = st;
+    s += (en - st + XP_CHUNK - 1) / XP_CHUNK;
+  }
   part[threadIdx.x] = s;
   __syncthreads();
   for (int o = 1; o < 1024; o <<= 1) {
@@ -273,18 +350,120 @@ __global__ void __launch_bounds__(1024) tile_ranges_kernel(int32_t* __restrict__
     __syncthreads();
   }
   uint32_t run = part[threadIdx.x] - s;
-  for (int t = b; t < e; t++) {
-    const uint32_t c = (uint32_t)sat[(t / gw) * sw + (t % gw)];
-    tile_ranges[2 * t] = run;
-    run += c;
-    tile_ranges[2 * t + 1] = run;
+  for (int r = b; r < e; r++) {
+    const uint32_t st = table_r[(size_t)r * n_chunks_r], en = table_r[(size_t)(r + 1) * n_chunks_r];
+    chunk_base[r] = run;
+    run += (en - st + XP_CHUNK - 1) / XP_CHUNK;
+  }
+  if (threadIdx.x == 1023) {
+    const uint32_t total = part[1023];
+    chunk_base[gh] = total;
+    row_start[gh] = table_r[(size_t)gh * n_chunks_r];
+    ctl->n_chunks_c = ctl->overflow ? 0u : total;
+    ctl->n_table_c = ctl->overflow ? 0u : total * (uint32_t)gw;
   }
 }
 
+// S3: column expansion.  Chunk g lies in row r (chunk_base[r] <= g < chunk_base[r+1]); its records cover
+// columns [x0, x1).  Table index of (r, tx, c) = gw * chunk_base[r] + tx * nchunk_r + c, so that a linear
+// exclusive scan of the table runs over tiles in row-major order and over chunks within a tile.
+template <bool kCount>
+__global__ void __launch_bounds__(32 * XP_MAX_WARPS) col_expand_kernel(
+    const uint2* __restrict__ row_rec, const uint32_t* __restrict__ row_start, const uint32_t* __restrict__ chunk_base,
+    const SortCtl* __restrict__ ctl, int gw, int gh, int warps_per_block, uint32_t* __restrict__ table_c,
+    uint32_t* __restrict__ sorted_ids) {
+  extern __shared__ uint32_t xp_smem[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t g = blockIdx.x * (uint32_t)warps_per_block + warp;
+  if (g >= ctl->n_chunks_c) return;
+  uint32_t* cnt = xp_smem + (size_t)warp * gw;
+  // row of this chunk: the last r with chunk_base[r] <= g
+  int lo_r = 0, hi_r = gh;  // invariant: chunk_base[lo_r] <= g < chunk_base[hi_r]
+  while (hi_r - lo_r > 1) {
+    const int mid = (lo_r + hi_r) >> 1;
+    if (chunk_base[mid] <= g) lo_r = mid; else hi_r = mid;
+  }
+  const int r = lo_r;
+  const uint32_t cb = chunk_base[r], nch = chunk_base[r + 1] - cb, c = g - cb;
+  const uint32_t j0 = row_start[r] + c * (uint32_t)XP_CHUNK;
+  const uint32_t j1 = min(j0 + (uint32_t)XP_CHUNK, row_start[r + 1]);
+  uint32_t* tab = table_c + (size_t)gw * cb + c;
+  for (int b = lane; b < gw; b += 32) cnt[b] = kCount ? 0u : tab[(size_t)b * nch];
+  __syncwarp();
+  for (uint32_t jb = j0; jb < j1; jb += 32) {
+    const uint32_t j = jb + lane;
+    uint32_t id = 0;
+    int lo = 0, hi = 0;
+    if (j < j1) {
+      const uint2 rec = row_rec[j];
+      id = rec.x;
+      lo = (int)(rec.y & 0xffffu); hi = (int)(rec.y >> 16);
+    }
+    int wlo, whi;
+    word_range(lo, hi, &wlo, &whi);
+    for (int w = wlo; w <= whi; w++) {
+      uint32_t col = transpose32(interval_bits(lo, hi, w), lane);
+      const int bin = 32 * w + lane;
+      if (kCount) {
+        if (col) cnt[bin] += __popc(col);
+      } else {
+        uint32_t p = col ? cnt[bin] : 0u;
+        const bool mine = col != 0;
+        while (__any_sync(0xffffffffu, col != 0)) {
+          const int src = col ? __ffs(col) - 1 : 0;
+          const uint32_t vid = __shfl_sync(0xffffffffu, id, src);
+          if (col) {
+            sorted_ids[p++] = vid;
+            col &= col - 1;
+          }
+        }
+        if (mine) cnt[bin] = p;
+      }
+    }
+  }
+  if (kCount) {
+    __syncwarp();
+    for (int b = lane; b < gw; b += 32) tab[(size_t)b * nch] = cnt[b];
+  }
+}
+
+// Tile ranges from the scanned column table: start(t) = scan value of (r, tx, chunk 0); a row without
+// records has no table entries and all its tiles start (and end) where the next row's first tile starts.
+__global__ void __launch_bounds__(256) tile_ranges_kernel(const uint32_t* __restrict__ table_c,
+                                                          const uint32_t* __restrict__ chunk_base,
+                                                          const SortCtl* __restrict__ ctl, int gw, int gh,
+                                                          uint32_t* __restrict__ tile_ranges) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  const int ntiles = gw * gh;
+  if (t >= ntiles) return;
+  if (ctl->overflow) {
+    tile_ranges[2 * t] = 0;
+    tile_ranges[2 * t + 1] = 0;
+    return;
+  }
+  uint32_t se[2];
+#pragma unroll
+  for (int q = 0; q < 2; q++) {
+    const int tt = t + q;
+    size_t idx;
+    if (tt >= ntiles) idx = ctl->n_table_c;
+    else {
+      const int r = tt / gw, tx = tt % gw;
+      const uint32_t cb = chunk_base[r], nch = chunk_base[r + 1] - cb;
+      idx = (size_t)gw * cb + (size_t)tx * nch;
+    }
+    se[q] = table_c[idx];
+  }
+  tile_ranges[2 * t] = se[0];
+  tile_ranges[2 * t + 1] = se[1];
+}
+
 struct Layout {
-  size_t ctl, keysA, valsA, keysB, valsB, block_sums, table, sat, tkA, tiA, tkB, tiB, total;
-  int nblkN_scan, nblkN_sort, nblkR_sort;
-  int tile_bits, tile_passes, bits_per_pass;
+  size_t ctl, keysA, valsA, keysB, valsB, table_n, sums, prect, table_r, row_start, chunk_base, row_rec, table_c, total;
+  int nblk_sort;          // blocks of a radix pass over N
+  uint32_t n_chunks_r;    // warps of the row expansion
+  uint32_t max_chunks_c;  // upper bound of the warps of the column expansion
+  uint32_t max_scan_blocks;
 };
 
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -292,30 +471,52 @@ inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 Layout make_layout(int64_t N, int gw, int gh, uint64_t Rcap) {
   Layout L;
   const size_t n = (size_t)N, r = (size_t)Rcap;
-  const int ntiles = gw * gh;
-  L.tile_bits = 1;
-  while ((1ll << L.tile_bits) < ntiles) L.tile_bits++;
-  L.tile_passes = (L.tile_bits + 7) / 8;
-  L.bits_per_pass = (L.tile_bits + L.tile_passes - 1) / L.tile_passes;
-  L.nblkN_scan = (int)((n + 255) / 256);
-  L.nblkN_sort = (int)((n + RS_TILE - 1) / RS_TILE);
-  L.nblkR_sort = (int)((r + RS_TILE - 1) / RS_TILE);
+  L.nblk_sort = (int)((n + RS_TILE - 1) / RS_TILE);
+  L.n_chunks_r = (uint32_t)((n + XP_CHUNK - 1) / XP_CHUNK);
+  L.max_chunks_c = (uint32_t)(r / XP_CHUNK + (size_t)gh);
+  const size_t tn = (size_t)RS_BINS * L.nblk_sort, tr = (size_t)gh * L.n_chunks_r, tc = (size_t)gw * L.max_chunks_c;
+  size_t tmax = tn > tr ? tn : tr;
+  if (tc > tmax) tmax = tc;
+  L.max_scan_blocks = (uint32_t)((tmax + SCAN_BLK - 1) / SCAN_BLK + 1);
   size_t o = 0;
   L.ctl = o; o = align256(o + sizeof(SortCtl));
   L.keysA = o; o = align256(o + 4 * n);
   L.valsA = o; o = align256(o + 4 * n);
   L.keysB = o; o = align256(o + 4 * n);
   L.valsB = o; o = align256(o + 4 * n);
-  L.block_sums = o; o = align256(o + 8 * (size_t)(L.nblkN_scan + 1));
-  const size_t tab = (size_t)RS_MAX_BINS * (size_t)(L.nblkN_sort > L.nblkR_sort ? L.nblkN_sort : L.nblkR_sort);
-  L.table = o; o = align256(o + 4 * (tab + 1));
-  L.sat = o; o = align256(o + 4 * (size_t)(gw + 1) * (gh + 1));
-  L.tkA = o; o = align256(o + 4 * r);
-  L.tiA = o; o = align256(o + 4 * r);
-  L.tkB = o; o = align256(o + (L.tile_passes > 1 ? 4 * r : 0));
-  L.tiB = o; o = align256(o + (L.tile_passes > 1 ? 4 * r : 0));
+  L.table_n = o; o = align256(o + 4 * (tn + 1));
+  L.sums = o; o = align256(o + 4 * (size_t)L.max_scan_blocks);
+  L.prect = o; o = align256(o + 8 * n);
+  L.table_r = o; o = align256(o + 4 * (tr + 1));
+  L.row_start = o; o = align256(o + 4 * (size_t)(gh + 1));
+  L.chunk_base = o; o = align256(o + 4 * (size_t)(gh + 1));
+  L.row_rec = o; o = align256(o + 8 * r);
+  L.table_c = o; o = align256(o + 4 * (tc + 1));
   L.total = o;
   return L;
+}
+
+// Warps per block of an expansion sweep with `bins` uint32 counters per warp in dynamic shared memory.
+inline int xp_warps(int bins) {
+  int w = (int)((160 * 1024) / ((size_t)bins * 4));
+  if (w > XP_MAX_WARPS) w = XP_MAX_WARPS;
+  if (w < 1) w = 1;
+  return w;
+}
+
+template <typename K>
+int xp_prepare(K kernel, size_t smem) {
+  if (smem > 48 * 1024) MG_CHECK_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  return MG_OK;
+}
+
+int scan_table(uint32_t* table, uint32_t n_static, const uint32_t* n_dev, uint32_t n_max, uint32_t* sums, cudaStream_t st) {
+  const uint32_t nb = (n_max + SCAN_BLK - 1) / SCAN_BLK;
+  const uint32_t grid = nb ? nb : 1;
+  scan_sums_kernel<<<grid, SCAN_THREADS, 0, st>>>(table, n_static, n_dev, sums);
+  scan_apply_kernel<<<grid, SCAN_THREADS, 0, st>>>(table, n_static, n_dev, sums);
+  MG_CHECK_LAUNCH();
+  return MG_OK;
 }
 
 }  // namespace
@@ -347,59 +548,67 @@ extern "C" int mg_bin_sort(const mg_camera* cam, int64_t N, const float* depths,
   SortCtl* ctl = (SortCtl*)(ws + L.ctl);
   uint32_t *keysA = (uint32_t*)(ws + L.keysA), *valsA = (uint32_t*)(ws + L.valsA);
   uint32_t *keysB = (uint32_t*)(ws + L.keysB), *valsB = (uint32_t*)(ws + L.valsB);
-  unsigned long long* block_sums = (unsigned long long*)(ws + L.block_sums);
-  uint32_t* table = (uint32_t*)(ws + L.table);
-  int32_t* sat = (int32_t*)(ws + L.sat);
-  uint32_t *tkA = (uint32_t*)(ws + L.tkA), *tiA = (uint32_t*)(ws + L.tiA);
-  uint32_t *tkB = (uint32_t*)(ws + L.tkB), *tiB = (uint32_t*)(ws + L.tiB);
-  const int sat_n = (gw + 1) * (gh + 1);
+  uint32_t *table_n = (uint32_t*)(ws + L.table_n), *sums = (uint32_t*)(ws + L.sums);
+  uint2* prect = (uint2*)(ws + L.prect);
+  uint32_t* table_r = (uint32_t*)(ws + L.table_r);
+  uint32_t *row_start = (uint32_t*)(ws + L.row_start), *chunk_base = (uint32_t*)(ws + L.chunk_base);
+  uint2* row_rec = (uint2*)(ws + L.row_rec);
+  uint32_t* table_c = (uint32_t*)(ws + L.table_c);
 
-  // (1) depth order of the N Gaussians: stable LSD radix sort of the fp32 depth bits, 4 x 8 bits
-  if (N > 0) {
-    depth_keys_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(N, depths, tiles_touched, keysA, valsA);
-    MG_CHECK_LAUNCH();
-    uint32_t *ki = keysA, *vi = valsA, *ko = keysB, *vo = valsB;
+  MG_CHECK_CUDA(cudaMemsetAsync(ctl, 0, sizeof(SortCtl), st));
+  if (N == 0) {
+    MG_CHECK_CUDA(cudaMemsetAsync(tile_ranges, 0, sizeof(uint32_t) * 2 * (size_t)gw * gh, st));
+    if (R_out_host) MG_CHECK_CUDA(cudaMemcpyAsync(R_out_host, &ctl->R, sizeof(uint64_t), cudaMemcpyDeviceToHost, st));
+    return MG_OK;
+  }
+
+  // S1: depth order of the N Gaussians (culled ones last), R, nvis, overflow flag
+  depth_keys_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(N, depths, tiles_touched, keysA, ctl);
+  ctl_finalize_kernel<<<1, 1, 0, st>>>(ctl, (unsigned long long)R_capacity);
+  MG_CHECK_LAUNCH();
+  {
+    uint32_t *ki = keysA, *vi = nullptr, *ko = keysB, *vo = valsB;
     for (int pass = 0; pass < 4; pass++) {
-      radix_pass_kernel<true, false><<<L.nblkN_sort, RS_THREADS, 0, st>>>(ki, vi, ko, vo, (uint32_t)N, nullptr, 8 * pass, 8, table, L.nblkN_sort);
-      table_scan_kernel<<<1, 1024, 0, st>>>(table, (size_t)256 * L.nblkN_sort);
-      radix_pass_kernel<false, true><<<L.nblkN_sort, RS_THREADS, 0, st>>>(ki, vi, ko, vo, (uint32_t)N, nullptr, 8 * pass, 8, table, L.nblkN_sort);
+      radix_pass_kernel<true><<<L.nblk_sort, RS_THREADS, 0, st>>>(ki, vi, ko, vo, (uint32_t)N, 8 * pass, table_n, L.nblk_sort);
+      if (int rc = scan_table(table_n, (uint32_t)(RS_BINS * L.nblk_sort), nullptr, (uint32_t)(RS_BINS * L.nblk_sort), sums, st)) return rc;
+      radix_pass_kernel<false><<<L.nblk_sort, RS_THREADS, 0, st>>>(ki, vi, ko, vo, (uint32_t)N, 8 * pass, table_n, L.nblk_sort);
       MG_CHECK_LAUNCH();
-      uint32_t* t = ki; ki = ko; ko = t;
-      t = vi; vi = vo; vo = t;
-    }
-    // after 4 passes the result is back in (keysA, valsA)
-    tt_block_sums_kernel<<<L.nblkN_scan, 256, 0, st>>>(N, valsA, tiles_touched, block_sums);
-    MG_CHECK_LAUNCH();
-  }
-  // (2) offsets of each Gaussian's run of keys; R and the overflow flag; clears the summed-area table
-  block_sums_scan_kernel<<<1, 1024, 0, st>>>(block_sums, N > 0 ? L.nblkN_scan : 0, R_capacity, ctl, sat, sat_n);
-  MG_CHECK_LAUNCH();
-  if (N > 0) {
-    // (3) duplication in depth order
-    uint32_t* first_ids = (L.tile_passes == 0) ? sorted_ids : tiA;
-    duplicate_kernel<<<L.nblkN_scan, 256, 0, st>>>(N, valsA, tiles_touched, (const int4*)rects, block_sums, ctl, gw, gh, tkA, first_ids, sat);
-    MG_CHECK_LAUNCH();
-    // (4) stable passes over the tile bits; the last one writes only the ids, to sorted_ids
-    if (R_capacity > 0) {
-      uint32_t *ki = tkA, *vi = tiA, *ko = tkB, *vo = tiB;
-      for (int pass = 0; pass < L.tile_passes; pass++) {
-        const bool last = pass == L.tile_passes - 1;
-        const int shift = pass * L.bits_per_pass;
-        radix_pass_kernel<true, false><<<L.nblkR_sort, RS_THREADS, 0, st>>>(ki, vi, ko, vo, (uint32_t)R_capacity, ctl, shift, L.bits_per_pass, table, L.nblkR_sort);
-        table_scan_kernel<<<1, 1024, 0, st>>>(table, ((size_t)1 << L.bits_per_pass) * L.nblkR_sort);
-        if (last)
-          radix_pass_kernel<false, false><<<L.nblkR_sort, RS_THREADS, 0, st>>>(ki, vi, nullptr, sorted_ids, (uint32_t)R_capacity, ctl, shift, L.bits_per_pass, table, L.nblkR_sort);
-        else
-          radix_pass_kernel<false, true><<<L.nblkR_sort, RS_THREADS, 0, st>>>(ki, vi, ko, vo, (uint32_t)R_capacity, ctl, shift, L.bits_per_pass, table, L.nblkR_sort);
-        MG_CHECK_LAUNCH();
-        uint32_t* t = ki; ki = ko; ko = t;
-        t = vi; vi = vo; vo = t;
-      }
+      ki = (pass & 1) ? keysA : keysB;
+      vi = (pass & 1) ? valsA : valsB;
+      ko = (pass & 1) ? keysB : keysA;
+      vo = (pass & 1) ? valsB : valsA;
     }
   }
-  // (5) tile ranges
-  tile_ranges_kernel<<<1, 1024, 0, st>>>(sat, gw, gh, ctl, tile_ranges);
-  MG_CHECK_LAUNCH();
+  const uint32_t* order = valsA;  // after 4 passes the result is in (keysA, valsA)
+
+  // S2: row expansion
+  {
+    const int wpb = xp_warps(gh);
+    const size_t smem = (size_t)wpb * gh * 4;
+    if (int rc = xp_prepare(row_expand_kernel<true>, smem)) return rc;
+    if (int rc = xp_prepare(row_expand_kernel<false>, smem)) return rc;
+    const unsigned grid = (L.n_chunks_r + wpb - 1) / wpb;
+    const uint32_t tr = (uint32_t)gh * L.n_chunks_r;
+    row_expand_kernel<true><<<grid, 32 * wpb, smem, st>>>(order, (const int4*)rects, ctl, gh, L.n_chunks_r, wpb, prect, table_r, row_rec);
+    if (int rc = scan_table(table_r, tr, nullptr, tr, sums, st)) return rc;
+    plan_kernel<<<1, 1024, 0, st>>>(table_r, L.n_chunks_r, gh, gw, row_start, chunk_base, ctl);
+    row_expand_kernel<false><<<grid, 32 * wpb, smem, st>>>(order, (const int4*)rects, ctl, gh, L.n_chunks_r, wpb, prect, table_r, row_rec);
+    MG_CHECK_LAUNCH();
+  }
+  // S3: column expansion and tile ranges
+  {
+    const int wpb = xp_warps(gw);
+    const size_t smem = (size_t)wpb * gw * 4;
+    if (int rc = xp_prepare(col_expand_kernel<true>, smem)) return rc;
+    if (int rc = xp_prepare(col_expand_kernel<false>, smem)) return rc;
+    const unsigned grid = (L.max_chunks_c + wpb - 1) / wpb;
+    const uint32_t tc_max = (uint32_t)gw * L.max_chunks_c;
+    col_expand_kernel<true><<<grid, 32 * wpb, smem, st>>>(row_rec, row_start, chunk_base, ctl, gw, gh, wpb, table_c, sorted_ids);
+    if (int rc = scan_table(table_c, 0, &ctl->n_table_c, tc_max, sums, st)) return rc;
+    col_expand_kernel<false><<<grid, 32 * wpb, smem, st>>>(row_rec, row_start, chunk_base, ctl, gw, gh, wpb, table_c, sorted_ids);
+    tile_ranges_kernel<<<(gw * gh + 255) / 256, 256, 0, st>>>(table_c, chunk_base, ctl, gw, gh, tile_ranges);
+    MG_CHECK_LAUNCH();
+  }
   if (R_out_host) MG_CHECK_CUDA(cudaMemcpyAsync(R_out_host, &ctl->R, sizeof(uint64_t), cudaMemcpyDeviceToHost, st));
   return MG_OK;
 }
