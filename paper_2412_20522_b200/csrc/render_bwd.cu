@@ -9,10 +9,13 @@
 // With q = alpha_i dL/dalpha_i (zero where the 0.99 clamp is active), the sums over pixels of
 // q, q dx, q dy, q dx^2, q dx dy, q dy^2 give dL/d(opacity, centre, conic) by a per-entry linear map.
 //
-// FP32-pipe and shuffle bound.  Same block geometry, staging and warp-level cull as the forward
-// kernel (render_common.cuh).  A lane sums its 4 pixels in registers; the 10 per-entry sums are then
-// reduced over the warp by a transposing butterfly (12 shuffles instead of 50) that leaves sum s in
-// lane pair s, and 10 lanes issue one red.global.add each.
+// FP32-pipe and shuffle bound.  Same geometry, staging and sub-block cull as the forward kernel
+// (render_common.cuh), walking each warp's strip from its largest n_contrib back to the front.
+//  * An entry with M = 0 leaves T and b unchanged and receives dL/dM only (Fig. 1): a
+//    warp-uniform branch with a third of the arithmetic, one plain butterfly and one atomic.
+//  * Otherwise a lane sums its (up to 4) pixels in registers; the 10 per-entry sums are reduced over
+//    the warp by a transposing butterfly (12 shuffles instead of 50) that leaves sum s in lane pair s,
+//    and 10 lanes issue one red.global.add each.
 #include "render_common.cuh"
 
 namespace {
@@ -23,7 +26,7 @@ struct BwdTargets {
   int offset[10];
 };
 
-// Sum each of 10 per-lane values over the 32 lanes.  Returns, in lanes whose slot (see rn_slot_of_lane)
+// Sum each of 10 per-lane values over the 32 lanes.  Returns, in lanes whose slot (see slot_of_lane)
 // is s >= 0, the total of v[s].
 __device__ __forceinline__ float transpose_reduce10(const float* v, int lane) {
   const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4, b1 = lane & 2;
@@ -68,36 +71,45 @@ __device__ __forceinline__ int slot_of_lane(int lane) {
   return idx < 0 ? -1 : 5 * b4 + idx;
 }
 
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+  for (int o = 16; o >= 1; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
 __global__ void __launch_bounds__(RN_THREADS) render_bwd_kernel(
     int W, int H, int gw, float bg0, float bg1, float bg2, const uint32_t* __restrict__ sorted_ids,
     const uint2* __restrict__ tile_ranges, const float2* __restrict__ means2d,
     const float4* __restrict__ conic_opacity, const float* __restrict__ rgb, const float* __restrict__ masks,
     const float* __restrict__ final_T, const uint32_t* __restrict__ n_contrib, const float* __restrict__ dL_dimage,
     BwdTargets tg) {
-  __shared__ RnRecord buf[2][RN_BATCH];
-  __shared__ uint32_t ids_sh[2][RN_BATCH];
-  __shared__ uint32_t wmax_sh[RN_THREADS / 32];
+  __shared__ RnRecord buf_all[RN_WARPS][32];
+  __shared__ uint32_t ids_all[RN_WARPS][32];
   const int tile = blockIdx.x;
   const int tx = tile % gw, ty = tile / gw;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  RnRecord* buf = buf_all[warp];
+  uint32_t* ids_sh = ids_all[warp];
   const uint2 range = tile_ranges[tile];
   const uint32_t* ids = sorted_ids + range.x;
 
-  const int px0 = tx * MG_TILE + 2 * (lane & 7), py0 = ty * MG_TILE + 8 * warp + 2 * (lane >> 3);
-  const float fx0 = (float)px0, fx1 = (float)(px0 + 1), fy0 = (float)py0, fy1 = (float)(py0 + 1);
-  const float X0 = (float)(tx * MG_TILE), Y0 = (float)(ty * MG_TILE + 8 * warp);
+  const int X0i = tx * MG_TILE, Y0i = ty * MG_TILE + 8 * warp;
+  const int px[2] = {X0i + (lane & 7), X0i + 8 + (lane & 7)};
+  const int py[2] = {Y0i + (lane >> 3), Y0i + 4 + (lane >> 3)};
+  const float fx[2] = {(float)px[0], (float)px[1]}, fy[2] = {(float)py[0], (float)py[1]};
+  const float X0 = (float)X0i, Y0 = (float)Y0i;
 
   // per-pixel state
   float T[4], gB[4], g0[4], g1[4], g2[4], tfg[4];
-  uint32_t last[4];
+  uint32_t last[4], sbmax[4];
   const size_t plane = (size_t)W * H;
-  uint32_t lmax = 0;
+  uint32_t wmax = 0;
 #pragma unroll
   for (int k = 0; k < 4; k++) {
-    const int px = px0 + (k & 1), py = py0 + (k >> 1);
+    const int x = px[k & 1], y = py[k >> 1];
     T[k] = 1.f; gB[k] = 0.f; g0[k] = g1[k] = g2[k] = 0.f; tfg[k] = 0.f; last[k] = 0;
-    if (px < W && py < H) {
-      const size_t pix = (size_t)py * W + px;
+    if (x < W && y < H) {
+      const size_t pix = (size_t)y * W + x;
       T[k] = final_T[pix];
       last[k] = n_contrib[pix];
       g0[k] = dL_dimage[pix];
@@ -105,16 +117,11 @@ __global__ void __launch_bounds__(RN_THREADS) render_bwd_kernel(
       g2[k] = dL_dimage[2 * plane + pix];
       tfg[k] = T[k] * (g0[k] * bg0 + g1[k] * bg1 + g2[k] * bg2);  // T_{N+1} g.c_bg
     }
-    lmax = max(lmax, last[k]);
+    sbmax[k] = __reduce_max_sync(0xffffffffu, last[k]);  // warp-uniform: last contributor of sub-block k
+    wmax = max(wmax, sbmax[k]);
   }
-  const uint32_t wmax = __reduce_max_sync(0xffffffffu, lmax);
-  if (lane == 0) wmax_sh[warp] = wmax;
-  __syncthreads();
-  uint32_t bmax = 0;
-#pragma unroll
-  for (int w = 0; w < RN_THREADS / 32; w++) bmax = max(bmax, wmax_sh[w]);
-  bmax = min(bmax, range.y - range.x);  // never walk past the tile's own list
-  if (bmax == 0) return;
+  wmax = min(wmax, range.y - range.x);  // never walk past the tile's own list
+  if (wmax == 0) return;                // warps do not synchronise with each other
 
   // where this lane's reduced sum goes
   const int slot = slot_of_lane(lane);
@@ -123,123 +130,134 @@ __global__ void __launch_bounds__(RN_THREADS) render_bwd_kernel(
 #pragma unroll
   for (int s = 0; s < 10; s++)
     if (slot == s) { tgt_base = tg.base[s]; tgt_stride = tg.stride[s]; tgt_off = tg.offset[s]; }
+  float* const dmask = tg.base[9];
 
-  const int n = (int)bmax;  // entries at positions > bmax are never visited
-  const int bstart = (n - 1) / RN_BATCH;
-  uint32_t id_next[2];
+  const int n = (int)wmax;  // entries at positions > wmax are never visited by this warp
+  const int bstart = ((n - 1) >> 5) << 5;
+  uint32_t id_cur = bstart + lane < n ? ids[bstart + lane] : 0u;
+  RnRaw raw_cur;
+  if (bstart + lane < n) raw_cur = rn_gather(id_cur, means2d, conic_opacity, rgb, masks);
+  uint32_t id_nxt = bstart >= 32 ? ids[bstart - 32 + lane] : 0u;
+
+  for (int base = bstart; base >= 0; base -= 32) {
+    RnRaw raw_nxt;
+    if (base >= 32) raw_nxt = rn_gather(id_nxt, means2d, conic_opacity, rgb, masks);
+    const uint32_t id_nxt2 = base >= 64 ? ids[base - 64 + lane] : 0u;
+
+    uint32_t m4 = 0;
+    __syncwarp();  // every lane is done reading the previous batch's records
+    if (base + lane < n) {
+      RnRecord rec = rn_make_record(raw_cur);
+      m4 = rn_subblock_mask(rec.a, rec.b, X0, Y0);
+      const uint32_t mypos = (uint32_t)(base + lane + 1);
 #pragma unroll
-  for (int s = 0; s < 2; s++) {
-    const int k = s * RN_THREADS + threadIdx.x;
-    const int i0 = bstart * RN_BATCH + k;
-    if (i0 < n) {
-      const uint32_t id = ids[i0];
-      ids_sh[0][k] = id;
-      buf[0][k] = rn_make_record(rn_gather(id, means2d, conic_opacity, rgb, masks));
+      for (int k = 0; k < 4; k++)
+        if (mypos > sbmax[k]) m4 &= ~(1u << k);
+      rec.c.w = __uint_as_float(m4);
+      buf[lane] = rec;
+      ids_sh[lane] = id_cur;
     }
-    const int i1 = (bstart - 1) * RN_BATCH + k;
-    id_next[s] = bstart >= 1 ? ids[i1] : 0u;
-  }
-  __syncthreads();
-
-  int cur = 0;
-  for (int b = bstart; b >= 0; b--) {
-    const int base = b * RN_BATCH;
-    const int cnt = min(RN_BATCH, n - base);
-    RnRaw raw[2];
-    uint32_t id_next2[2];
-#pragma unroll
-    for (int s = 0; s < 2; s++) {
-      const int k = s * RN_THREADS + threadIdx.x;
-      if (b >= 1) raw[s] = rn_gather(id_next[s], means2d, conic_opacity, rgb, masks);
-      id_next2[s] = b >= 2 ? ids[(b - 2) * RN_BATCH + k] : 0u;
+    __syncwarp();  // records visible to the whole warp
+    uint32_t todo = __ballot_sync(0xffffffffu, m4 != 0);
+    float4 nra, nrb, nrc;
+    if (todo) {
+      const int j = 31 - __clz(todo);
+      nra = buf[j].a; nrb = buf[j].b; nrc = buf[j].c;
     }
-
-    const RnRecord* rec = buf[cur];
-    for (int c0 = ((cnt - 1) >> 5) << 5; c0 >= 0; c0 -= 32) {
-      const int j = c0 + lane;
-      bool keep = false;
-      if (j < cnt && (uint32_t)(base + j + 1) <= wmax) {
-        const float4 ra = rec[j].a, rb = rec[j].b;
-        keep = rn_max_e_over_strip(ra, rb, X0, Y0) >= RN_LOG2_ALPHA_MIN - RN_CULL_SLACK;
+    while (todo) {
+      const int jj = 31 - __clz(todo);
+      todo &= ~(1u << jj);
+      const float4 ra = nra, rb = nrb, rc = nrc;
+      if (todo) {
+        const int j = 31 - __clz(todo);
+        nra = buf[j].a; nrb = buf[j].b; nrc = buf[j].c;
       }
-      uint32_t todo = __ballot_sync(0xffffffffu, keep);
-      while (todo) {
-        const int bit = 31 - __clz(todo);
-        todo &= ~(1u << bit);
-        const int jj = c0 + bit;
-        const float4 ra = rec[jj].a, rb = rec[jj].b;
-        const float lo = rb.y;
-        float dx[2], dy[2], e[4];
-        rn_eval_quad(ra, rb, fx0, fx1, fy0, fy1, dx, dy, e);
-        uint32_t pass = rn_filter_quad(e, lo);
-        const uint32_t pos = (uint32_t)(base + jj + 1);
-#pragma unroll
-        for (int k = 0; k < 4; k++)
-          if (pos > last[k]) pass &= ~(1u << k);
-        if (!__any_sync(0xffffffffu, pass != 0)) continue;
+      const uint32_t sb = __float_as_uint(rc.w);
+      const float lo = rb.y, m = rb.z;
+      const uint32_t pos = (uint32_t)(base + jj + 1);
+      const RnPartial p = rn_partial(ra, rb, fx, fy);
 
-        const float4 rc = rec[jj].c;
-        const float m = rb.z;
-        float S = 0.f, Sx = 0.f, Sy = 0.f, Sxx = 0.f, Sxy = 0.f, Syy = 0.f;
-        float dr = 0.f, dg = 0.f, db = 0.f, dm = 0.f;
+      if (m == 0.f) {
+        // masked entry: a = 0, T_i = T_{i+1}, b unchanged; only dL/dM = sum alpha X (Eq. 18)
+        float dm = 0.f;
 #pragma unroll
         for (int k = 0; k < 4; k++) {
-          if (pass >> k & 1u) {
-            const float raw_alpha = rn_ex2(e[k]);
-            const float alpha = fminf(MG_ALPHA_MAX, raw_alpha);
-            const float a = m * alpha;
-            const float oma = 1.f - a;
-            const float inv = __frcp_rn(oma);
-            const float Ti = T[k] * inv;
-            const float gc = g0[k] * rc.x + g1[k] * rc.y + g2[k] * rc.z;
-            const float X = Ti * (gc - gB[k]) - tfg[k] * inv;
-            dm = fmaf(alpha, X, dm);
-            const float wgt = a * Ti;
-            dr = fmaf(wgt, g0[k], dr);
-            dg = fmaf(wgt, g1[k], dg);
-            db = fmaf(wgt, g2[k], db);
-            gB[k] = fmaf(a, gc, oma * gB[k]);
-            T[k] = Ti;
-            if (raw_alpha <= MG_ALPHA_MAX) {
-              const float q = alpha * (m * X);
-              const float ddx = dx[k & 1], ddy = dy[k >> 1];
-              const float qx = q * ddx, qy = q * ddy;
-              S += q; Sx += qx; Sy += qy;
-              Sxx = fmaf(qx, ddx, Sxx);
-              Sxy = fmaf(qx, ddy, Sxy);
-              Syy = fmaf(qy, ddy, Syy);
+          if ((sb >> k) & 1u) {
+            const float e = rn_eval(p, ra.w, k);
+            if (rn_filter(e, lo) && pos <= last[k]) {
+              const float alpha = fminf(MG_ALPHA_MAX, rn_ex2(e));
+              const float gc = g0[k] * rc.x + g1[k] * rc.y + g2[k] * rc.z;
+              const float X = T[k] * (gc - gB[k]) - tfg[k];
+              dm = fmaf(alpha, X, dm);
             }
           }
         }
-        // per-entry linear map: true conic (A,B,C) = (-2 ln2 A2, -ln2 B2, -2 ln2 C2)
-        float v[10];
-        v[0] = RN_LN2 * (2.f * ra.z * Sx + ra.w * Sy);   // dL/dmean2d.x = -(A Sx + B Sy)
-        v[1] = RN_LN2 * (ra.w * Sx + 2.f * rb.x * Sy);   // dL/dmean2d.y = -(B Sx + C Sy)
-        v[2] = -0.5f * Sxx;                              // dL/dA
-        v[3] = -Sxy;                                     // dL/dB
-        v[4] = -0.5f * Syy;                              // dL/dC
-        v[5] = S * rb.w;                                 // dL/do = sum q / o
-        v[6] = dr; v[7] = dg; v[8] = db;
-        v[9] = dm;
-        const float total = transpose_reduce10(v, lane);
-        if (slot >= 0 && total != 0.f) {
-          const uint32_t id = ids_sh[cur][jj];
-          atomicAdd(tgt_base + (size_t)id * tgt_stride + tgt_off, total);
+        if (__any_sync(0xffffffffu, dm != 0.f)) {
+          const float total = warp_sum(dm);
+          if (lane == 0) atomicAdd(dmask + ids_sh[jj], total);
+        }
+        continue;
+      }
+
+      float S = 0.f, Sx = 0.f, Sy = 0.f, Sxx = 0.f, Sxy = 0.f, Syy = 0.f;
+      float dr = 0.f, dg = 0.f, db = 0.f, dm = 0.f;
+      bool contrib = false;
+#pragma unroll
+      for (int k = 0; k < 4; k++) {
+        if ((sb >> k) & 1u) {
+          const float e = rn_eval(p, ra.w, k);
+          const bool pass = rn_filter(e, lo) && pos <= last[k];
+          if (__any_sync(0xffffffffu, pass)) {
+            contrib = true;
+            if (pass) {
+              const float raw_alpha = rn_ex2(e);
+              const float alpha = fminf(MG_ALPHA_MAX, raw_alpha);
+              const float a = m * alpha;
+              const float oma = 1.f - a;
+              const float inv = rn_rcp(oma);
+              const float Ti = T[k] * inv;
+              const float gc = g0[k] * rc.x + g1[k] * rc.y + g2[k] * rc.z;
+              const float X = Ti * (gc - gB[k]) - tfg[k] * inv;
+              dm = fmaf(alpha, X, dm);
+              const float wgt = a * Ti;
+              dr = fmaf(wgt, g0[k], dr);
+              dg = fmaf(wgt, g1[k], dg);
+              db = fmaf(wgt, g2[k], db);
+              gB[k] = fmaf(a, gc, oma * gB[k]);
+              T[k] = Ti;
+              if (raw_alpha <= MG_ALPHA_MAX) {
+                const float q = alpha * (m * X);
+                const float ddx = p.dx[k & 1], ddy = p.dy[k >> 1];
+                const float qx = q * ddx, qy = q * ddy;
+                S += q; Sx += qx; Sy += qy;
+                Sxx = fmaf(qx, ddx, Sxx);
+                Sxy = fmaf(qx, ddy, Sxy);
+                Syy = fmaf(qy, ddy, Syy);
+              }
+            }
+          }
         }
       }
-    }
-
-#pragma unroll
-    for (int s = 0; s < 2; s++) {
-      const int k = s * RN_THREADS + threadIdx.x;
-      if (b >= 1) {
-        ids_sh[cur ^ 1][k] = id_next[s];
-        buf[cur ^ 1][k] = rn_make_record(raw[s]);
+      if (!contrib) continue;
+      // per-entry linear map: true conic (A,B,C) = (-2 ln2 A2, -ln2 B2, -2 ln2 C2)
+      float v[10];
+      v[0] = RN_LN2 * (2.f * ra.z * Sx + ra.w * Sy);   // dL/dmean2d.x = -(A Sx + B Sy)
+      v[1] = RN_LN2 * (ra.w * Sx + 2.f * rb.x * Sy);   // dL/dmean2d.y = -(B Sx + C Sy)
+      v[2] = -0.5f * Sxx;                              // dL/dA
+      v[3] = -Sxy;                                     // dL/dB
+      v[4] = -0.5f * Syy;                              // dL/dC
+      v[5] = S * rb.w;                                 // dL/do = sum q / o
+      v[6] = dr; v[7] = dg; v[8] = db;
+      v[9] = dm;
+      const float total = transpose_reduce10(v, lane);
+      if (slot >= 0 && total != 0.f) {
+        const uint32_t id = ids_sh[jj];
+        atomicAdd(tgt_base + (size_t)id * tgt_stride + tgt_off, total);
       }
-      id_next[s] = id_next2[s];
     }
-    cur ^= 1;
-    __syncthreads();
+    raw_cur = raw_nxt;
+    id_cur = id_nxt;
+    id_nxt = id_nxt2;
   }
 }
 

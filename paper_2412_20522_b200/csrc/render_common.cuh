@@ -1,12 +1,18 @@
 // render_common.cuh -- pieces shared by the forward and backward blend kernels.
 //
-// Geometry of a block: one 16x16 tile, 64 threads = 2 warps.  A warp owns a 16x8
-// pixel strip; a lane owns a 2x2 pixel quad, so the per-entry record read from shared memory and the
-// row/column partial products are shared by 4 pixels, and (backward) 4 pixels are summed in
-// registers before any cross-lane reduction.
+// Geometry: one block per 16x16 tile, 64 threads = 2 warps that never synchronise with
+// each other.  A warp owns a 16x8 pixel strip, seen as four 8x4 SUB-BLOCKS (k = 2*by + bx); a lane owns
+// one pixel of each sub-block, at the same offset (lane & 7, lane >> 3).  A splat that is small against
+// the strip then activates one or two sub-blocks, whose 32 pixels are exactly the 32 lanes, instead of a
+// few lanes of every instruction.
 //
-// Per-entry record staged in shared memory (3 x float4).  The conic is pre-scaled into the log2
-// domain and the opacity folded in as an offset, so that
+// Each warp stages its tile's list itself, 32 entries at a time (lane j fetches entry j): ids two
+// batches ahead and attributes one batch ahead in registers, the current batch as 48-byte records in
+// shared memory.  While a lane still holds its entry in registers it computes a 4-bit mask of the
+// sub-blocks the entry can reach (exact maximum of the concave exponent over each 8x4 box); entries
+// that reach no live sub-block are dropped by a ballot, the others are walked in list order.
+//
+// Record: the conic is pre-scaled into the log2 domain and the opacity folded in as an offset, so that
 //     log2(alpha) = e = lo + A2 dx^2 + B2 dx dy + C2 dy^2,   d = mean2d - pixel,
 // and the alpha filter of the method (power > 0 or alpha < 1/255 => skip) becomes two compares on e
 // BEFORE any exponential is taken:  e > lo  or  e < log2(1/255).
@@ -14,16 +20,16 @@
 #include "mg_common.cuh"
 
 #define RN_THREADS 64
-#define RN_BATCH 128
+#define RN_WARPS (RN_THREADS / 32)
 #define RN_LOG2E 1.4426950408889634f
 #define RN_LN2 0.6931471805599453f
 #define RN_LOG2_ALPHA_MIN -7.994353436858858f  // log2(1/255)
-#define RN_CULL_SLACK 1e-3f                    // warp-level cull keeps entries within 2^-10 of the threshold
+#define RN_CULL_SLACK 1e-3f                    // the sub-block cull keeps entries within 2^-10 of the threshold
 
 struct RnRecord {
   float4 a;  // mx, my, A2, B2
-  float4 b;  // C2, lo, mask, 1/o (backward) or unused
-  float4 c;  // r, g, b, unused
+  float4 b;  // C2, lo, mask, 1/o
+  float4 c;  // r, g, b, sub-block mask (bits)
 };
 
 __device__ __forceinline__ float rn_ex2(float x) {
@@ -34,6 +40,11 @@ __device__ __forceinline__ float rn_ex2(float x) {
 __device__ __forceinline__ float rn_lg2(float x) {
   float y;
   asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ float rn_rcp(float x) {
+  float y;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
 
@@ -64,12 +75,13 @@ __device__ __forceinline__ RnRecord rn_make_record(const RnRaw& v) {
   return r;
 }
 
-// Largest e over the pixel rectangle [X0, X0+15] x [Y0, Y0+7] (e is a concave quadratic in d; its
+// Largest e over the pixel rectangle [xlo, xhi] x [ylo, yhi] (e is a concave quadratic in d; its
 // maximum over a box whose interior misses the centre lies on an edge next to the centre).
-__device__ __forceinline__ float rn_max_e_over_strip(const float4& ra, const float4& rb, float X0, float Y0) {
+__device__ __forceinline__ float rn_max_e_over_box(const float4& ra, const float4& rb, float xlo, float xhi, float ylo,
+                                                   float yhi) {
   const float A2 = ra.z, B2 = ra.w, C2 = rb.x, lo = rb.y;
-  const float dxlo = ra.x - (X0 + 15.f), dxhi = ra.x - X0;
-  const float dylo = ra.y - (Y0 + 7.f), dyhi = ra.y - Y0;
+  const float dxlo = ra.x - xhi, dxhi = ra.x - xlo;
+  const float dylo = ra.y - yhi, dyhi = ra.y - ylo;
   const float dxc = fminf(fmaxf(0.f, dxlo), dxhi), dyc = fminf(fmaxf(0.f, dylo), dyhi);
   // edge dx = dxc: best dy
   const float dy1 = fminf(fmaxf(__fdividef(-B2 * dxc, 2.f * C2), dylo), dyhi);
@@ -80,29 +92,41 @@ __device__ __forceinline__ float rn_max_e_over_strip(const float4& ra, const flo
   return fmaxf(e1, e2);
 }
 
-// e = log2(alpha) at the four pixels of a quad (k = 2*row + col).  Explicit rounding intrinsics: the
-// forward and the backward kernel must take bit-identical alpha-filter decisions, so the compiler
-// is not allowed to contract or reassociate this differently in the two kernels.
-__device__ __forceinline__ void rn_eval_quad(const float4& ra, const float4& rb, float fx0, float fx1, float fy0,
-                                             float fy1, float* dx, float* dy, float* e) {
-  dx[0] = __fsub_rn(ra.x, fx0);
-  dx[1] = __fsub_rn(ra.x, fx1);
-  dy[0] = __fsub_rn(ra.y, fy0);
-  dy[1] = __fsub_rn(ra.y, fy1);
-  const float adx0 = __fmul_rn(ra.z, dx[0]), adx1 = __fmul_rn(ra.z, dx[1]);
-  const float cyp0 = __fmaf_rn(__fmul_rn(rb.x, dy[0]), dy[0], rb.y);
-  const float cyp1 = __fmaf_rn(__fmul_rn(rb.x, dy[1]), dy[1], rb.y);
-  e[0] = __fmaf_rn(dx[0], __fmaf_rn(ra.w, dy[0], adx0), cyp0);
-  e[1] = __fmaf_rn(dx[1], __fmaf_rn(ra.w, dy[0], adx1), cyp0);
-  e[2] = __fmaf_rn(dx[0], __fmaf_rn(ra.w, dy[1], adx0), cyp1);
-  e[3] = __fmaf_rn(dx[1], __fmaf_rn(ra.w, dy[1], adx1), cyp1);
+// Bit k set = the entry can pass the alpha filter somewhere in sub-block k of the strip at (X0, Y0).
+__device__ __forceinline__ uint32_t rn_subblock_mask(const float4& ra, const float4& rb, float X0, float Y0) {
+  uint32_t m = 0;
+#pragma unroll
+  for (int k = 0; k < 4; k++) {
+    const float xlo = X0 + 8.f * (k & 1), ylo = Y0 + 4.f * (k >> 1);
+    if (rn_max_e_over_box(ra, rb, xlo, xlo + 7.f, ylo, ylo + 3.f) >= RN_LOG2_ALPHA_MIN - RN_CULL_SLACK) m |= 1u << k;
+  }
+  return m;
+}
+
+// Per-entry partial products of e for a lane's pixel columns (bx = 0, 1) and rows (by = 0, 1).
+struct RnPartial {
+  float dx[2], dy[2], adx[2], cyp[2];
+};
+
+// Explicit rounding intrinsics: the forward and the backward kernel must take bit-identical
+// alpha-filter decisions, so the compiler is not allowed to contract or reassociate this differently
+// in the two kernels.
+__device__ __forceinline__ RnPartial rn_partial(const float4& ra, const float4& rb, const float* fx, const float* fy) {
+  RnPartial p;
+#pragma unroll
+  for (int i = 0; i < 2; i++) {
+    p.dx[i] = __fsub_rn(ra.x, fx[i]);
+    p.dy[i] = __fsub_rn(ra.y, fy[i]);
+    p.adx[i] = __fmul_rn(ra.z, p.dx[i]);
+    p.cyp[i] = __fmaf_rn(__fmul_rn(rb.x, p.dy[i]), p.dy[i], rb.y);
+  }
+  return p;
+}
+
+// e = log2(alpha) at the lane's pixel of sub-block k.
+__device__ __forceinline__ float rn_eval(const RnPartial& p, float B2, int k) {
+  return __fmaf_rn(p.dx[k & 1], __fmaf_rn(B2, p.dy[k >> 1], p.adx[k & 1]), p.cyp[k >> 1]);
 }
 
 // The alpha filter on the exponent: power > 0 (e > lo) or alpha < 1/255 => the pair is skipped.
-__device__ __forceinline__ uint32_t rn_filter_quad(const float* e, float lo) {
-  uint32_t pass = 0;
-#pragma unroll
-  for (int k = 0; k < 4; k++)
-    if (e[k] <= lo && e[k] >= RN_LOG2_ALPHA_MIN) pass |= 1u << k;
-  return pass;
-}
+__device__ __forceinline__ bool rn_filter(float e, float lo) { return e <= lo && e >= RN_LOG2_ALPHA_MIN; }

@@ -2,14 +2,15 @@
 // Eq. 3-4: C += M_i alpha_i T_i c_i,  T_{i+1} = (1 - M_i alpha_i) T_i;
 // Eq. 9-10: image = C + T_{N+1} c_bg.  Thresholds: DESIGN.md readings 1-5.
 //
-// FP32-pipe bound (no dense contraction on this path, so no tensor cores).  Design:
-//  * 2 warps per tile, a 2x2 pixel quad per lane (render_common.cuh);
-//  * list entries gathered one batch ahead into registers, converted to log2-domain records and
-//    staged in double-buffered shared memory: one barrier per batch of 128 entries;
-//  * per warp, 32 entries at a time are tested against the warp's 16x8 strip (exact maximum of the
-//    concave exponent over the strip) and only the survivors are evaluated per pixel;
-//  * the alpha filter is two compares on the exponent, the exponential is taken only for pairs
-//    that pass; a warp leaves the loop when all its pixels have stopped.
+// FP32-pipe bound (no dense contraction on this path, so no tensor cores).  Design (render_common.cuh):
+//  * 2 independent warps per tile, each a 16x8 strip of four 8x4 sub-blocks, one pixel of each per lane;
+//  * per warp, 32 list entries at a time: attributes gathered one batch ahead, a 4-bit sub-block reach
+//    mask per entry (lanes = entries), a ballot, then the surviving entries in list order;
+//  * per surviving entry only the reachable, still-live sub-blocks are evaluated; the alpha filter is two
+//    compares on the exponent, the exponential is taken only for pairs that pass;
+//  * an entry with M = 0 changes neither C nor T: for it only the last-contributor index is
+//    updated -- a warp-uniform branch, since M belongs to the entry;
+//  * a warp leaves when all its pixels have stopped.
 #include "render_common.cuh"
 
 namespace {
@@ -19,121 +20,128 @@ __global__ void __launch_bounds__(RN_THREADS) render_fwd_kernel(
     const uint2* __restrict__ tile_ranges, const float2* __restrict__ means2d,
     const float4* __restrict__ conic_opacity, const float* __restrict__ rgb, const float* __restrict__ masks,
     float* __restrict__ image, float* __restrict__ final_T, uint32_t* __restrict__ n_contrib) {
-  __shared__ RnRecord buf[2][RN_BATCH];
+  __shared__ RnRecord buf_all[RN_WARPS][32];
   const int tile = blockIdx.x;
   const int tx = tile % gw, ty = tile / gw;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  RnRecord* buf = buf_all[warp];
   const uint2 range = tile_ranges[tile];
   const int n = (int)(range.y - range.x);
   const uint32_t* ids = sorted_ids + range.x;
 
-  // quad of this lane
-  const int px0 = tx * MG_TILE + 2 * (lane & 7), py0 = ty * MG_TILE + 8 * warp + 2 * (lane >> 3);
-  const float fx0 = (float)px0, fx1 = (float)(px0 + 1), fy0 = (float)py0, fy1 = (float)(py0 + 1);
-  const float X0 = (float)(tx * MG_TILE), Y0 = (float)(ty * MG_TILE + 8 * warp);
+  // pixels of this lane: (px[bx], py[by]), sub-block k = 2*by + bx
+  const int X0i = tx * MG_TILE, Y0i = ty * MG_TILE + 8 * warp;
+  const int px[2] = {X0i + (lane & 7), X0i + 8 + (lane & 7)};
+  const int py[2] = {Y0i + (lane >> 3), Y0i + 4 + (lane >> 3)};
+  const float fx[2] = {(float)px[0], (float)px[1]}, fy[2] = {(float)py[0], (float)py[1]};
+  const float X0 = (float)X0i, Y0 = (float)Y0i;
 
-  float T[4] = {1.f, 1.f, 1.f, 1.f};
-  float Cr[4] = {0.f, 0.f, 0.f, 0.f}, Cg[4] = {0.f, 0.f, 0.f, 0.f}, Cb[4] = {0.f, 0.f, 0.f, 0.f};
-  uint32_t last[4] = {0u, 0u, 0u, 0u};
-  // bit k set = pixel k still running (k = 2*row + col).  Pixels outside the image never run.
-  uint32_t live = 0;
-  if (px0 < W && py0 < H) live |= 1u;
-  if (px0 + 1 < W && py0 < H) live |= 2u;
-  if (px0 < W && py0 + 1 < H) live |= 4u;
-  if (px0 + 1 < W && py0 + 1 < H) live |= 8u;
-  bool warp_done = !__any_sync(0xffffffffu, live != 0);
-
-  const int nbatches = (n + RN_BATCH - 1) / RN_BATCH;
-  // prologue: batch 0 -> buf[0]; ids of batch 1 -> registers
-  uint32_t id_next[2];
+  float T[4], Cr[4], Cg[4], Cb[4];
+  uint32_t last[4];
+  uint32_t live = 0;  // bit k set = pixel k still running.  Pixels outside the image never run.
 #pragma unroll
-  for (int s = 0; s < 2; s++) {
-    const int k = s * RN_THREADS + threadIdx.x;
-    if (k < n) buf[0][k] = rn_make_record(rn_gather(ids[k], means2d, conic_opacity, rgb, masks));
-    const int k1 = RN_BATCH + k;
-    id_next[s] = k1 < n ? ids[k1] : 0u;
+  for (int k = 0; k < 4; k++) {
+    T[k] = 1.f; Cr[k] = Cg[k] = Cb[k] = 0.f; last[k] = 0u;
+    if (px[k & 1] < W && py[k >> 1] < H) live |= 1u << k;
   }
-  __syncthreads();
-
-  int cur = 0;
-  for (int b = 0; b < nbatches; b++) {
-    const int base = b * RN_BATCH;
-    const int cnt = min(RN_BATCH, n - base);
-    // issue the gathers of batch b+1 and the id loads of batch b+2 before computing on batch b
-    RnRaw raw[2];
-    uint32_t id_next2[2];
+  uint32_t live_sb = 0;  // warp-uniform: bit k set = sub-block k has a running pixel
 #pragma unroll
-    for (int s = 0; s < 2; s++) {
-      const int k = s * RN_THREADS + threadIdx.x;
-      if (base + RN_BATCH + k < n) raw[s] = rn_gather(id_next[s], means2d, conic_opacity, rgb, masks);
-      const int k2 = base + 2 * RN_BATCH + k;
-      id_next2[s] = k2 < n ? ids[k2] : 0u;
-    }
+  for (int k = 0; k < 4; k++)
+    if (__any_sync(0xffffffffu, (live >> k) & 1u)) live_sb |= 1u << k;
 
-    if (!warp_done) {
-      const RnRecord* rec = buf[cur];
-      for (int c0 = 0; c0 < cnt; c0 += 32) {
-        // warp-level cull of 32 entries against this warp's strip
-        const int j = c0 + lane;
-        bool keep = false;
-        if (j < cnt) {
-          const float4 ra = rec[j].a, rb = rec[j].b;
-          keep = rn_max_e_over_strip(ra, rb, X0, Y0) >= RN_LOG2_ALPHA_MIN - RN_CULL_SLACK;
+  if (n > 0 && live_sb) {
+    // prologue: attributes of batch 0 and ids of batch 1 into registers
+    RnRaw raw_cur;
+    if (lane < n) raw_cur = rn_gather(ids[lane], means2d, conic_opacity, rgb, masks);
+    uint32_t id_nxt = 32 + lane < n ? ids[32 + lane] : 0u;
+
+    for (int base = 0; base < n; base += 32) {
+      // issue the gathers of the next batch and the id loads of the one after before computing
+      RnRaw raw_nxt;
+      if (base + 32 + lane < n) raw_nxt = rn_gather(id_nxt, means2d, conic_opacity, rgb, masks);
+      const uint32_t id_nxt2 = base + 64 + lane < n ? ids[base + 64 + lane] : 0u;
+
+      uint32_t m4 = 0;
+      __syncwarp();  // every lane is done reading the previous batch's records
+      if (base + lane < n) {
+        RnRecord rec = rn_make_record(raw_cur);
+        m4 = rn_subblock_mask(rec.a, rec.b, X0, Y0) & live_sb;
+        rec.c.w = __uint_as_float(m4);
+        buf[lane] = rec;
+      }
+      __syncwarp();  // records visible to the whole warp
+      uint32_t todo = __ballot_sync(0xffffffffu, m4 != 0);
+      // software pipeline: the record of the next survivor is loaded while the current one is blended
+      float4 nra, nrb, nrc;
+      if (todo) {
+        const int j = __ffs(todo) - 1;
+        nra = buf[j].a; nrb = buf[j].b; nrc = buf[j].c;
+      }
+      while (todo) {
+        const int jj = __ffs(todo) - 1;
+        todo &= todo - 1;
+        const float4 ra = nra, rb = nrb, rc = nrc;
+        if (todo) {
+          const int j = __ffs(todo) - 1;
+          nra = buf[j].a; nrb = buf[j].b; nrc = buf[j].c;
         }
-        uint32_t todo = __ballot_sync(0xffffffffu, keep);
-        while (todo) {
-          const int jj = c0 + __ffs(todo) - 1;
-          todo &= todo - 1;
-          const float4 ra = rec[jj].a, rb = rec[jj].b;
-          const float lo = rb.y;
-          float dx[2], dy[2], e[4];
-          rn_eval_quad(ra, rb, fx0, fx1, fy0, fy1, dx, dy, e);
-          uint32_t pass = rn_filter_quad(e, lo);
-          pass &= live;
-          if (__any_sync(0xffffffffu, pass != 0)) {
-            const float4 rc = rec[jj].c;
-            const uint32_t pos = (uint32_t)(base + jj + 1);
+        const uint32_t sb = __float_as_uint(rc.w) & live_sb;
+        const float lo = rb.y, m = rb.z;
+        const uint32_t pos = (uint32_t)(base + jj + 1);
+        const RnPartial p = rn_partial(ra, rb, fx, fy);
+        if (m == 0.f) {
+          // masked entry: a = 0, so C and T are unchanged and the pixel cannot stop here
 #pragma unroll
-            for (int k = 0; k < 4; k++) {
-              if (pass >> k & 1u) {
-                const float alpha = fminf(MG_ALPHA_MAX, rn_ex2(e[k]));
-                const float a = rb.z * alpha;
-                const float Tn = T[k] * (1.f - a);
-                if (Tn < MG_T_MIN) {
-                  live &= ~(1u << k);  // stop: this entry is neither blended nor counted
-                } else {
-                  const float w = a * T[k];
-                  Cr[k] = fmaf(w, rc.x, Cr[k]);
-                  Cg[k] = fmaf(w, rc.y, Cg[k]);
-                  Cb[k] = fmaf(w, rc.z, Cb[k]);
-                  T[k] = Tn;
-                  last[k] = pos;
+          for (int k = 0; k < 4; k++) {
+            if ((sb >> k) & 1u) {
+              const float e = rn_eval(p, ra.w, k);
+              if (rn_filter(e, lo) && ((live >> k) & 1u)) last[k] = pos;
+            }
+          }
+        } else {
+#pragma unroll
+          for (int k = 0; k < 4; k++) {
+            if ((sb >> k) & 1u) {
+              const float e = rn_eval(p, ra.w, k);
+              const bool pass = rn_filter(e, lo) && ((live >> k) & 1u);
+              if (__any_sync(0xffffffffu, pass)) {
+                if (pass) {
+                  const float alpha = fminf(MG_ALPHA_MAX, rn_ex2(e));
+                  const float a = m * alpha;
+                  const float Tn = T[k] * (1.f - a);
+                  if (Tn < MG_T_MIN) {
+                    live &= ~(1u << k);  // stop: this entry is neither blended nor counted
+                  } else {
+                    const float w = a * T[k];
+                    Cr[k] = fmaf(w, rc.x, Cr[k]);
+                    Cg[k] = fmaf(w, rc.y, Cg[k]);
+                    Cb[k] = fmaf(w, rc.z, Cb[k]);
+                    T[k] = Tn;
+                    last[k] = pos;
+                  }
                 }
               }
             }
           }
         }
-        if (!__any_sync(0xffffffffu, live != 0)) { warp_done = true; break; }
       }
-    }
-
-    // publish batch b+1 into the other buffer
+      // refresh the live sub-blocks once per batch
+      live_sb = 0;
 #pragma unroll
-    for (int s = 0; s < 2; s++) {
-      const int k = s * RN_THREADS + threadIdx.x;
-      if (base + RN_BATCH + k < n) buf[cur ^ 1][k] = rn_make_record(raw[s]);
-      id_next[s] = id_next2[s];
+      for (int k = 0; k < 4; k++)
+        if (__any_sync(0xffffffffu, (live >> k) & 1u)) live_sb |= 1u << k;
+      if (!live_sb) break;
+      raw_cur = raw_nxt;
+      id_nxt = id_nxt2;
     }
-    cur ^= 1;
-    if (__syncthreads_and(warp_done)) break;
   }
 
   const size_t plane = (size_t)W * H;
 #pragma unroll
   for (int k = 0; k < 4; k++) {
-    const int px = px0 + (k & 1), py = py0 + (k >> 1);
-    if (px < W && py < H) {
-      const size_t pix = (size_t)py * W + px;
+    const int x = px[k & 1], y = py[k >> 1];
+    if (x < W && y < H) {
+      const size_t pix = (size_t)y * W + x;
       image[pix] = fmaf(T[k], bg0, Cr[k]);
       image[plane + pix] = fmaf(T[k], bg1, Cg[k]);
       image[2 * plane + pix] = fmaf(T[k], bg2, Cb[k]);
