@@ -31,8 +31,10 @@ if ROOT not in sys.path:
 FLOP_PAIR = 13        # per pair evaluation: 2 sub, 6 quadratic form, mul, min, 2 compares (+1 MUFU not counted)
 FLOP_BLEND_FWD = 11   # per blend, forward
 FLOP_BLEND_BWD = 59   # per blend, backward (49 + 10 adds of the per-entry reduction)
-KERNELS_PER_STEP = {"preprocess": 1, "bin_sort_fixed": 17, "bin_sort_per_tile_pass": 3, "render_fwd": 1,
-                    "render_bwd": 1, "preprocess_bwd": 1}
+# kernels of libmg launched per step (memsets and copies not counted): bin_sort = depth keys + ctl + 4 x (count,
+# 2 scan, scatter) + row expansion (count, 2 scan, plan, emit) + column expansion (count, 2 scan, emit, ranges)
+KERNELS_PER_STEP = {"preprocess": 1, "bin_sort": 2 + 4 * 4 + 5 + 5, "render_fwd": 1, "render_bwd": 1,
+                    "preprocess_bwd": 1}
 
 
 def work_counts(cfg):
@@ -118,6 +120,18 @@ def oracle_sample(cfg, n_tiles_target=None, seed=0):
             f"on those tiles ({t2 - t1:.1f}+{t3 - t2:.1f}+{t4 - t3:.1f} s) + {frac:.4f} x (preprocess {t1 - t0:.1f} s + "
             f"preprocess_bwd {t5 - t4:.1f} s)")
     return blends, seconds, info
+
+
+def max_over_ranks(value, world, device):
+    """MAX over ranks of a per-rank scalar (the contract's multi-GPU timing rule).  nccl on cuda, gloo on cpu."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
 
 
 def n_threads():
@@ -228,10 +242,7 @@ def main():
     total_ms = ev[0][0].elapsed_time(ev[-1][5])
     per_call = {n: float(np.mean([ev[s][i].elapsed_time(ev[s][i + 1]) for s in range(args.steps)])) for i, n in enumerate(names)}
     assert int(fr.R_host[1]) == R
-    if world > 1:
-        t = torch.tensor([total_ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, world, "cuda")
     ms_step = total_ms / args.steps
 
     # ---- e2e: host buffers, H2D of every input + D2H of image and gradients inside the timed region
@@ -261,10 +272,7 @@ def main():
     e1.record()
     barrier()
     e2e_ms = e0.elapsed_time(e1) / args.e2e_steps
-    if world > 1:
-        t = torch.tensor([e2e_ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
+    e2e_ms = max_over_ranks(e2e_ms, world, "cuda")
 
     if rank != 0:
         if world > 1:
@@ -299,8 +307,7 @@ def main():
         cpu = {"value": b / sec, "unit": "blends/s", "cores": n_threads(), "kind": "oracle", "sample": info}
 
     gw, gh = mg.grid(cam)
-    tile_passes = 1 if gw * gh <= 256 else (2 if gw * gh <= 65536 else 3)
-    launches = args.steps * (1 + KERNELS_PER_STEP["bin_sort_fixed"] + 3 * tile_passes + 1 + 1 + 1)
+    launches = args.steps * sum(KERNELS_PER_STEP.values())
     line = {"metric": "gaussian_pixel_blends_per_s", "value": value, "unit": "blends/s", "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",

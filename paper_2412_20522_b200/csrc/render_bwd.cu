@@ -18,6 +18,10 @@
 //    and 10 lanes issue one red.global.add each.
 #include "render_common.cuh"
 
+#ifndef RN_BWD_MINB
+#define RN_BWD_MINB 10  // minimum resident blocks per SM asked of ptxas (register budget)
+#endif
+
 namespace {
 
 struct BwdTargets {
@@ -77,18 +81,20 @@ __device__ __forceinline__ float warp_sum(float v) {
   return v;
 }
 
-__global__ void __launch_bounds__(RN_THREADS) render_bwd_kernel(
+__global__ void __launch_bounds__(RN_THREADS, RN_BWD_MINB) render_bwd_kernel(
     int W, int H, int gw, float bg0, float bg1, float bg2, const uint32_t* __restrict__ sorted_ids,
     const uint2* __restrict__ tile_ranges, const float2* __restrict__ means2d,
     const float4* __restrict__ conic_opacity, const float* __restrict__ rgb, const float* __restrict__ masks,
     const float* __restrict__ final_T, const uint32_t* __restrict__ n_contrib, const float* __restrict__ dL_dimage,
     BwdTargets tg) {
   __shared__ RnRecord buf_all[RN_WARPS][32];
+  __shared__ RnStage stage_all[RN_WARPS];
   __shared__ uint32_t ids_all[RN_WARPS][32];
   const int tile = blockIdx.x;
   const int tx = tile % gw, ty = tile / gw;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   RnRecord* buf = buf_all[warp];
+  RnStage* stage = &stage_all[warp];
   uint32_t* ids_sh = ids_all[warp];
   const uint2 range = tile_ranges[tile];
   const uint32_t* ids = sorted_ids + range.x;
@@ -134,20 +140,18 @@ __global__ void __launch_bounds__(RN_THREADS) render_bwd_kernel(
 
   const int n = (int)wmax;  // entries at positions > wmax are never visited by this warp
   const int bstart = ((n - 1) >> 5) << 5;
+  // prologue: gather of the last batch in flight, ids of the one before it in a register
   uint32_t id_cur = bstart + lane < n ? ids[bstart + lane] : 0u;
-  RnRaw raw_cur;
-  if (bstart + lane < n) raw_cur = rn_gather(id_cur, means2d, conic_opacity, rgb, masks);
+  if (bstart + lane < n) rn_stage_issue(stage, lane, id_cur, means2d, conic_opacity, rgb, masks);
+  rn_cp_async_commit();
   uint32_t id_nxt = bstart >= 32 ? ids[bstart - 32 + lane] : 0u;
 
   for (int base = bstart; base >= 0; base -= 32) {
-    RnRaw raw_nxt;
-    if (base >= 32) raw_nxt = rn_gather(id_nxt, means2d, conic_opacity, rgb, masks);
-    const uint32_t id_nxt2 = base >= 64 ? ids[base - 64 + lane] : 0u;
-
+    rn_cp_async_wait_all();  // this lane's entry of the current batch has landed
+    __syncwarp();            // every lane is done reading the previous batch's records
     uint32_t m4 = 0;
-    __syncwarp();  // every lane is done reading the previous batch's records
     if (base + lane < n) {
-      RnRecord rec = rn_make_record(raw_cur);
+      RnRecord rec = rn_make_record(rn_stage_read(stage, lane));
       m4 = rn_subblock_mask(rec.a, rec.b, X0, Y0);
       const uint32_t mypos = (uint32_t)(base + lane + 1);
 #pragma unroll
@@ -157,21 +161,17 @@ __global__ void __launch_bounds__(RN_THREADS) render_bwd_kernel(
       buf[lane] = rec;
       ids_sh[lane] = id_cur;
     }
+    // gather of the next batch (towards the front) and id load of the one after
+    if (base >= 32) rn_stage_issue(stage, lane, id_nxt, means2d, conic_opacity, rgb, masks);
+    rn_cp_async_commit();
+    id_cur = id_nxt;
+    id_nxt = base >= 64 ? ids[base - 64 + lane] : 0u;
     __syncwarp();  // records visible to the whole warp
     uint32_t todo = __ballot_sync(0xffffffffu, m4 != 0);
-    float4 nra, nrb, nrc;
-    if (todo) {
-      const int j = 31 - __clz(todo);
-      nra = buf[j].a; nrb = buf[j].b; nrc = buf[j].c;
-    }
     while (todo) {
       const int jj = 31 - __clz(todo);
       todo &= ~(1u << jj);
-      const float4 ra = nra, rb = nrb, rc = nrc;
-      if (todo) {
-        const int j = 31 - __clz(todo);
-        nra = buf[j].a; nrb = buf[j].b; nrc = buf[j].c;
-      }
+      const float4 ra = buf[jj].a, rb = buf[jj].b, rc = buf[jj].c;
       const uint32_t sb = __float_as_uint(rc.w);
       const float lo = rb.y, m = rb.z;
       const uint32_t pos = (uint32_t)(base + jj + 1);
@@ -255,9 +255,6 @@ __global__ void __launch_bounds__(RN_THREADS) render_bwd_kernel(
         atomicAdd(tgt_base + (size_t)id * tgt_stride + tgt_off, total);
       }
     }
-    raw_cur = raw_nxt;
-    id_cur = id_nxt;
-    id_nxt = id_nxt2;
   }
 }
 

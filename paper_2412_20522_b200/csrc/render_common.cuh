@@ -7,8 +7,8 @@
 // few lanes of every instruction.
 //
 // Each warp stages its tile's list itself, 32 entries at a time (lane j fetches entry j): ids two
-// batches ahead and attributes one batch ahead in registers, the current batch as 48-byte records in
-// shared memory.  While a lane still holds its entry in registers it computes a 4-bit mask of the
+// batches ahead in a register, attributes one batch ahead by cp.async into shared memory (no registers
+// held across the blend loop), the current batch as 48-byte records in shared memory.  While a lane still holds its entry in registers it computes a 4-bit mask of the
 // sub-blocks the entry can reach (exact maximum of the concave exponent over each 8x4 box); entries
 // that reach no live sub-block are dropped by a ballot, the others are walked in list order.
 //
@@ -54,16 +54,44 @@ struct RnRaw {  // attributes of one list entry as gathered from global memory
   float r, g, b, m;
 };
 
-__device__ __forceinline__ RnRaw rn_gather(uint32_t id, const float2* __restrict__ means2d,
-                                           const float4* __restrict__ conic_opacity, const float* __restrict__ rgb,
-                                           const float* __restrict__ masks) {
+// Per-warp landing zone of the asynchronous gather (cp.async, LDGSTS): lane j's entry lands in slot j of
+// each array, so the gather of the next batch costs no registers while the current batch is blended.
+// A slot is written and read by the same lane only.
+struct RnStage {
+  float4 co[32];
+  float2 m2[32];
+  float rgb[32][3];
+  float m[32];
+};
+
+__device__ __forceinline__ void rn_cp_async(void* smem_dst, const void* gmem_src, int bytes) {
+  const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+  if (bytes == 16) asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
+  else if (bytes == 8) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gmem_src) : "memory");
+  else asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void rn_cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void rn_cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+__device__ __forceinline__ void rn_stage_issue(RnStage* s, int lane, uint32_t id, const float2* __restrict__ means2d,
+                                               const float4* __restrict__ conic_opacity, const float* __restrict__ rgb,
+                                               const float* __restrict__ masks) {
+  rn_cp_async(&s->co[lane], conic_opacity + id, 16);
+  rn_cp_async(&s->m2[lane], means2d + id, 8);
+  rn_cp_async(&s->rgb[lane][0], rgb + 3 * (size_t)id, 4);
+  rn_cp_async(&s->rgb[lane][1], rgb + 3 * (size_t)id + 1, 4);
+  rn_cp_async(&s->rgb[lane][2], rgb + 3 * (size_t)id + 2, 4);
+  rn_cp_async(&s->m[lane], masks + id, 4);
+}
+
+__device__ __forceinline__ RnRaw rn_stage_read(const RnStage* s, int lane) {
   RnRaw v;
-  v.m2 = __ldg(means2d + id);
-  v.co = __ldg(conic_opacity + id);
-  v.r = __ldg(rgb + 3 * (size_t)id);
-  v.g = __ldg(rgb + 3 * (size_t)id + 1);
-  v.b = __ldg(rgb + 3 * (size_t)id + 2);
-  v.m = __ldg(masks + id);
+  v.m2 = s->m2[lane];
+  v.co = s->co[lane];
+  v.r = s->rgb[lane][0];
+  v.g = s->rgb[lane][1];
+  v.b = s->rgb[lane][2];
+  v.m = s->m[lane];
   return v;
 }
 

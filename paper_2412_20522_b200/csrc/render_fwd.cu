@@ -4,7 +4,7 @@
 //
 // FP32-pipe bound (no dense contraction on this path, so no tensor cores).  Design (render_common.cuh):
 //  * 2 independent warps per tile, each a 16x8 strip of four 8x4 sub-blocks, one pixel of each per lane;
-//  * per warp, 32 list entries at a time: attributes gathered one batch ahead, a 4-bit sub-block reach
+//  * per warp, 32 list entries at a time: attributes gathered one batch ahead (cp.async), a 4-bit sub-block reach
 //    mask per entry (lanes = entries), a ballot, then the surviving entries in list order;
 //  * per surviving entry only the reachable, still-live sub-blocks are evaluated; the alpha filter is two
 //    compares on the exponent, the exponential is taken only for pairs that pass;
@@ -13,18 +13,24 @@
 //  * a warp leaves when all its pixels have stopped.
 #include "render_common.cuh"
 
+#ifndef RN_FWD_MINB
+#define RN_FWD_MINB 14  // minimum resident blocks per SM asked of ptxas (register budget)
+#endif
+
 namespace {
 
-__global__ void __launch_bounds__(RN_THREADS) render_fwd_kernel(
+__global__ void __launch_bounds__(RN_THREADS, RN_FWD_MINB) render_fwd_kernel(
     int W, int H, int gw, float bg0, float bg1, float bg2, const uint32_t* __restrict__ sorted_ids,
     const uint2* __restrict__ tile_ranges, const float2* __restrict__ means2d,
     const float4* __restrict__ conic_opacity, const float* __restrict__ rgb, const float* __restrict__ masks,
     float* __restrict__ image, float* __restrict__ final_T, uint32_t* __restrict__ n_contrib) {
   __shared__ RnRecord buf_all[RN_WARPS][32];
+  __shared__ RnStage stage_all[RN_WARPS];
   const int tile = blockIdx.x;
   const int tx = tile % gw, ty = tile / gw;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   RnRecord* buf = buf_all[warp];
+  RnStage* stage = &stage_all[warp];
   const uint2 range = tile_ranges[tile];
   const int n = (int)(range.y - range.x);
   const uint32_t* ids = sorted_ids + range.x;
@@ -50,41 +56,31 @@ __global__ void __launch_bounds__(RN_THREADS) render_fwd_kernel(
     if (__any_sync(0xffffffffu, (live >> k) & 1u)) live_sb |= 1u << k;
 
   if (n > 0 && live_sb) {
-    // prologue: attributes of batch 0 and ids of batch 1 into registers
-    RnRaw raw_cur;
-    if (lane < n) raw_cur = rn_gather(ids[lane], means2d, conic_opacity, rgb, masks);
+    // prologue: gather of batch 0 in flight, ids of batch 1 in a register
+    if (lane < n) rn_stage_issue(stage, lane, ids[lane], means2d, conic_opacity, rgb, masks);
+    rn_cp_async_commit();
     uint32_t id_nxt = 32 + lane < n ? ids[32 + lane] : 0u;
 
     for (int base = 0; base < n; base += 32) {
-      // issue the gathers of the next batch and the id loads of the one after before computing
-      RnRaw raw_nxt;
-      if (base + 32 + lane < n) raw_nxt = rn_gather(id_nxt, means2d, conic_opacity, rgb, masks);
-      const uint32_t id_nxt2 = base + 64 + lane < n ? ids[base + 64 + lane] : 0u;
-
+      rn_cp_async_wait_all();  // this lane's entry of the current batch has landed
+      __syncwarp();            // every lane is done reading the previous batch's records
       uint32_t m4 = 0;
-      __syncwarp();  // every lane is done reading the previous batch's records
       if (base + lane < n) {
-        RnRecord rec = rn_make_record(raw_cur);
+        RnRecord rec = rn_make_record(rn_stage_read(stage, lane));
         m4 = rn_subblock_mask(rec.a, rec.b, X0, Y0) & live_sb;
         rec.c.w = __uint_as_float(m4);
         buf[lane] = rec;
       }
+      // gather of the next batch and id load of the one after, in flight during the blend loop
+      if (base + 32 + lane < n) rn_stage_issue(stage, lane, id_nxt, means2d, conic_opacity, rgb, masks);
+      rn_cp_async_commit();
+      id_nxt = base + 64 + lane < n ? ids[base + 64 + lane] : 0u;
       __syncwarp();  // records visible to the whole warp
       uint32_t todo = __ballot_sync(0xffffffffu, m4 != 0);
-      // software pipeline: the record of the next survivor is loaded while the current one is blended
-      float4 nra, nrb, nrc;
-      if (todo) {
-        const int j = __ffs(todo) - 1;
-        nra = buf[j].a; nrb = buf[j].b; nrc = buf[j].c;
-      }
       while (todo) {
         const int jj = __ffs(todo) - 1;
         todo &= todo - 1;
-        const float4 ra = nra, rb = nrb, rc = nrc;
-        if (todo) {
-          const int j = __ffs(todo) - 1;
-          nra = buf[j].a; nrb = buf[j].b; nrc = buf[j].c;
-        }
+        const float4 ra = buf[jj].a, rb = buf[jj].b, rc = buf[jj].c;
         const uint32_t sb = __float_as_uint(rc.w) & live_sb;
         const float lo = rb.y, m = rb.z;
         const uint32_t pos = (uint32_t)(base + jj + 1);
@@ -131,9 +127,8 @@ __global__ void __launch_bounds__(RN_THREADS) render_fwd_kernel(
       for (int k = 0; k < 4; k++)
         if (__any_sync(0xffffffffu, (live >> k) & 1u)) live_sb |= 1u << k;
       if (!live_sb) break;
-      raw_cur = raw_nxt;
-      id_nxt = id_nxt2;
     }
+    rn_cp_async_wait_all();
   }
 
   const size_t plane = (size_t)W * H;

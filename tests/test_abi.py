@@ -47,10 +47,12 @@ def test_workspace_bytes_host_logic(lib):
     small = binding.mg_workspace_bytes(1000, 128, 128, 3000)
     big = binding.mg_workspace_bytes(1000, 128, 128, 3_000_000)
     assert 0 < small < big
-    # <= 256 tiles: one tile pass, so no second ping-pong buffer (8 B per key); more tiles: 16 B per key
-    one = binding.mg_workspace_bytes(0, 256, 256, 1_000_000)
-    two = binding.mg_workspace_bytes(0, 512, 512, 1_000_000)
-    assert one < 8.5e6 and 16e6 <= two < 17e6
+    # layout of bin_sort v2: 8 B of row records per key of capacity, 24 B per Gaussian (depth keys, ids, packed
+    # rects), plus the count tables (a few % of that)
+    keys_only = binding.mg_workspace_bytes(0, 512, 512, 1_000_000)
+    assert 8e6 <= keys_only < 8.6e6
+    both = binding.mg_workspace_bytes(1_000_000, 512, 512, 1_000_000)
+    assert 24e6 <= both - keys_only < 26e6
 
 
 def test_invalid_arguments_are_rejected_without_a_gpu(lib):
