@@ -34,7 +34,7 @@ FLOP_BLEND_BWD = 59   # per blend, backward (49 + 10 adds of the per-entry reduc
 # kernels of libmg launched per step (memsets and copies not counted): bin_sort = depth keys + ctl + 4 x (count,
 # 2 scan, scatter) + row expansion (count, 2 scan, plan, emit) + column expansion (count, 2 scan, emit, ranges)
 KERNELS_PER_STEP = {"preprocess": 1, "bin_sort": 2 + 4 * 4 + 5 + 5, "render_fwd": 1, "render_bwd": 1,
-                    "preprocess_bwd": 1}
+                    "preprocess_bwd": 2}
 
 
 def work_counts(cfg):

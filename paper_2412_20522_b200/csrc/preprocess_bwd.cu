@@ -2,49 +2,141 @@
 // The paper gives no formulas for this step ("We modify the CUDA rasterization code of 3DGS",
 // PAPER.md:156); it is the chain rule of DESIGN.md O1-O8, hand-derived here in reverse mode.  The
 // oracle obtains the same quantity by forward-mode dual numbers, so the two derivations are independent.
-// HBM-bound: one thread per Gaussian; 236 B of inputs + 36 B of upstream gradients in, 236 B out.
+// HBM-bound: one thread per Gaussian; 236 B of inputs + 36 B of upstream gradients in, 236 B out;
+// the 192-byte SH rows (in and out) are staged through shared memory so that global accesses coalesce.
 #include "mg_common.cuh"
 
 namespace {
 
+// SH rows move through shared memory: a warp's 32 rows are contiguous in global memory (32 x 3K floats),
+// so they are loaded and stored with fully coalesced 128-bit accesses by flat position, and each thread
+// reads / writes its own row in shared memory (row stride chosen so that 128-bit shared accesses of 8
+// consecutive lanes cover all banks).  Rows of culled Gaussians are not read; their gradients are zeros.
 template <int D>
-__global__ void __launch_bounds__(128) preprocess_bwd_kernel(
-    mg_camera cam, int64_t N, const float* __restrict__ means, const float* __restrict__ log_scales,
-    const float* __restrict__ quats, const float* __restrict__ opacity_logits, const float* __restrict__ sh,
-    const int32_t* __restrict__ radii, const uint8_t* __restrict__ clamped, const float2* __restrict__ dL_dmeans2d,
-    const float* __restrict__ dL_dconic, const float* __restrict__ dL_dopacity, const float* __restrict__ dL_drgb,
-    float* __restrict__ dL_dmeans, float* __restrict__ dL_dlog_scales, float4* __restrict__ dL_dquats,
-    float* __restrict__ dL_dopacity_logits, float* __restrict__ dL_dsh) {
-  constexpr int K = (D + 1) * (D + 1);
-  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= N) return;
-  float* gsh = dL_dsh + i * (3 * K);
-  if (radii[i] <= 0) {  // culled: exact zeros everywhere
-    dL_dmeans[3 * i] = dL_dmeans[3 * i + 1] = dL_dmeans[3 * i + 2] = 0.f;
-    dL_dlog_scales[3 * i] = dL_dlog_scales[3 * i + 1] = dL_dlog_scales[3 * i + 2] = 0.f;
-    dL_dquats[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-    dL_dopacity_logits[i] = 0.f;
-    if ((3 * K) % 4 == 0) {
-#pragma unroll
-      for (int j = 0; j < 3 * K / 4; j++) reinterpret_cast<float4*>(gsh)[j] = make_float4(0.f, 0.f, 0.f, 0.f);
-    } else {
-#pragma unroll
-      for (int j = 0; j < 3 * K; j++) gsh[j] = 0.f;
-    }
-    return;
-  }
-  const float* R = cam.R;
-  const float px = means[3 * i], py = means[3 * i + 1], pz = means[3 * i + 2];
-  const float4 q = __ldg(reinterpret_cast<const float4*>(quats) + i);
-  const double s0 = exp((double)log_scales[3 * i]), s1 = exp((double)log_scales[3 * i + 1]), s2 = exp((double)log_scales[3 * i + 2]);
-  const float o = 1.f / (1.f + expf(-opacity_logits[i]));
-  const float2 gm = dL_dmeans2d[i];
-  const float gA = dL_dconic[3 * i], gB = dL_dconic[3 * i + 1], gC = dL_dconic[3 * i + 2];
-  const uint32_t cl = clamped[i];
-  float gcol[3];
-#pragma unroll
-  for (int k = 0; k < 3; k++) gcol[k] = (cl >> k & 1u) ? 0.f : dL_drgb[3 * i + k];
+struct ShRowLayout {
+  static constexpr int K = (D + 1) * (D + 1);
+  static constexpr int RK = 3 * K;                  // floats per row
+  static constexpr bool VEC = (RK % 4) == 0;        // D = 1, 3
+  static constexpr int STRIDE = VEC ? (((RK / 4) % 2) ? RK : RK + 4) : ((RK % 2) ? RK : RK + 1);
+};
 
+#ifndef PB_H
+#define PB_H float
+#endif
+
+// Tail of the reverse pass, from dL/dU on.  Given dL/dU the remaining chain is sums of products of
+// well-conditioned quantities, so it runs in H (fp32 by default; -DPB_H=double to compare).
+struct GeoGrads {
+  float dls[3];
+  float4 dq;
+  float dm[3];
+};
+
+template <typename H>
+__device__ __forceinline__ GeoGrads geometry_tail(const H* Rd, bool xcl, bool ycl, H dU00, H dU01, H dU02, H dU10, H dU11, H dU12, H M00, H M01, H M02, H M10, H M11, H M12, H M20, H M21, H M22, H T00, H T01, H T02, H T10, H T11, H T12, H r00, H r01, H r02, H r10, H r11, H r12, H r20, H r21, H r22, H s0, H s1, H s2, H qw, H qx, H qy, H qz, H qinv, H fxd, H fyd, H iz, H tx, H ty, H xz, H yz, H gmx, H gmy, H dmx, H dmy, H dmz) {
+  GeoGrads out;
+  // U = T M:  dT = dU M^T,  dM = T^T dU
+  const H dT00 = dU00 * M00 + dU01 * M01 + dU02 * M02, dT01 = dU00 * M10 + dU01 * M11 + dU02 * M12, dT02 = dU00 * M20 + dU01 * M21 + dU02 * M22;
+  const H dT10 = dU10 * M00 + dU11 * M01 + dU12 * M02, dT11 = dU10 * M10 + dU11 * M11 + dU12 * M12, dT12 = dU10 * M20 + dU11 * M21 + dU12 * M22;
+  const H dM00 = T00 * dU00 + T10 * dU10, dM01 = T00 * dU01 + T10 * dU11, dM02 = T00 * dU02 + T10 * dU12;
+  const H dM10 = T01 * dU00 + T11 * dU10, dM11 = T01 * dU01 + T11 * dU11, dM12 = T01 * dU02 + T11 * dU12;
+  const H dM20 = T02 * dU00 + T12 * dU10, dM21 = T02 * dU01 + T12 * dU11, dM22 = T02 * dU02 + T12 * dU12;
+  // M = Rot diag(s)
+  const H ds0 = dM00 * r00 + dM10 * r10 + dM20 * r20;
+  const H ds1 = dM01 * r01 + dM11 * r11 + dM21 * r21;
+  const H ds2 = dM02 * r02 + dM12 * r12 + dM22 * r22;
+  out.dls[0] = (float)(ds0 * s0);
+  out.dls[1] = (float)(ds1 * s1);
+  out.dls[2] = (float)(ds2 * s2);
+  const H dr00 = dM00 * s0, dr01 = dM01 * s1, dr02 = dM02 * s2;
+  const H dr10 = dM10 * s0, dr11 = dM11 * s1, dr12 = dM12 * s2;
+  const H dr20 = dM20 * s0, dr21 = dM21 * s1, dr22 = dM22 * s2;
+  // Rot(unit quaternion)
+  const H dqw = (H)2. * (-qz * dr01 + qy * dr02 + qz * dr10 - qx * dr12 - qy * dr20 + qx * dr21);
+  const H dqx = (H)2. * (qy * dr01 + qz * dr02 + qy * dr10 - (H)2. * qx * dr11 - qw * dr12 + qz * dr20 + qw * dr21 - (H)2. * qx * dr22);
+  const H dqy = (H)2. * (-(H)2. * qy * dr00 + qx * dr01 + qw * dr02 + qx * dr10 + qz * dr12 - qw * dr20 + qz * dr21 - (H)2. * qy * dr22);
+  const H dqz = (H)2. * (-(H)2. * qz * dr00 - qw * dr01 + qx * dr02 + qw * dr10 - (H)2. * qz * dr11 + qy * dr12 + qx * dr20 + qy * dr21);
+  // through q / |q|
+  const H qdot = qw * dqw + qx * dqx + qy * dqy + qz * dqz;
+  out.dq = make_float4((float)((dqw - qw * qdot) * qinv), (float)((dqx - qx * qdot) * qinv), (float)((dqy - qy * qdot) * qinv), (float)((dqz - qz * qdot) * qinv));
+  // T = J W
+  const H dJ00 = dT00 * Rd[0] + dT01 * Rd[1] + dT02 * Rd[2];
+  const H dJ02 = dT00 * Rd[6] + dT01 * Rd[7] + dT02 * Rd[8];
+  const H dJ11 = dT10 * Rd[3] + dT11 * Rd[4] + dT12 * Rd[5];
+  const H dJ12 = dT10 * Rd[6] + dT11 * Rd[7] + dT12 * Rd[8];
+  // J(t) and the projected centre
+  const H iz2 = iz * iz;
+  H dtx = gmx * fxd * iz, dty = gmy * fyd * iz;
+  H dtz = -(dJ00 * fxd + dJ11 * fyd) * iz2 - ((H)gmx * fxd * tx + (H)gmy * fyd * ty) * iz2;
+  if (xcl) dtz += dJ02 * fxd * xz * iz2;  // J02 = -fx L / z with L = +-limx
+  else { dtx += -dJ02 * fxd * iz2; dtz += dJ02 * (H)2. * fxd * tx * iz2 * iz; }
+  if (ycl) dtz += dJ12 * fyd * yz * iz2;
+  else { dty += -dJ12 * fyd * iz2; dtz += dJ12 * (H)2. * fyd * ty * iz2 * iz; }
+  // t = R p + t_cam
+  const H dmx_g = Rd[0] * dtx + Rd[3] * dty + Rd[6] * dtz;
+  const H dmy_g = Rd[1] * dtx + Rd[4] * dty + Rd[7] * dtz;
+  const H dmz_g = Rd[2] * dtx + Rd[5] * dty + Rd[8] * dtz;
+  out.dm[0] = (float)((H)dmx + dmx_g);
+  out.dm[1] = (float)((H)dmy + dmy_g);
+  out.dm[2] = (float)((H)dmz + dmz_g);
+  return out;
+}
+
+constexpr int PB_THREADS = 128;
+#ifndef PB_MINB
+#define PB_MINB 4
+#endif
+#ifndef PB_G
+#define PB_G double
+#endif
+
+// Kernel 1 of 2: colour.  dL/dsh, and the part of dL/dmean that flows through the view direction (written to
+// dL_dmeans; kernel 2 adds the geometric part).  fp32, light on registers, HBM-bound.
+template <int D>
+__global__ void __launch_bounds__(PB_THREADS) preprocess_bwd_sh_kernel(
+    mg_camera cam, int64_t N, const float* __restrict__ means, const float* __restrict__ sh,
+    const int32_t* __restrict__ radii, const uint8_t* __restrict__ clamped, const float* __restrict__ dL_drgb,
+    float* __restrict__ dL_dmeans, float* __restrict__ dL_dsh) {
+  typedef ShRowLayout<D> L;
+  constexpr int K = L::K, RK = L::RK, STRIDE = L::STRIDE;
+  __shared__ __align__(16) float rows_all[PB_THREADS / 32][32 * STRIDE];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  float* wrow = rows_all[warp];
+  float* myrow = wrow + lane * STRIDE;
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t g0 = i - lane;                              // first Gaussian of this warp
+  const int nrows = (int)max((int64_t)0, min((int64_t)32, N - g0));
+  const bool vis = i < N && radii[i] > 0;
+  const uint32_t vmask = __ballot_sync(0xffffffffu, vis);
+  // this thread's own small inputs first, so that they are in flight together with the rows
+  float px = 0.f, py = 0.f, pz = 0.f, gcol[3] = {0.f, 0.f, 0.f};
+  if (vis) {
+    px = means[3 * i]; py = means[3 * i + 1]; pz = means[3 * i + 2];
+    const uint32_t cl = clamped[i];
+#pragma unroll
+    for (int k = 0; k < 3; k++) gcol[k] = (cl >> k & 1u) ? 0.f : dL_drgb[3 * i + k];
+  }
+  // coalesced load of the visible rows
+  if (nrows > 0) {
+    if (L::VEC) {
+      const float4* src = reinterpret_cast<const float4*>(sh + g0 * RK);
+#pragma unroll
+      for (int k = 0; k < RK / 4; k++) {
+        const int f = k * 32 + lane, g = f / (RK / 4), c = f % (RK / 4);
+        if (g < nrows && ((vmask >> g) & 1u)) *reinterpret_cast<float4*>(wrow + g * STRIDE + 4 * c) = __ldg(src + f);
+      }
+    } else {
+      const float* src = sh + g0 * RK;
+#pragma unroll
+      for (int k = 0; k < RK; k++) {
+        const int f = k * 32 + lane, g = f / RK, c = f % RK;
+        if (g < nrows && ((vmask >> g) & 1u)) wrow[g * STRIDE + c] = __ldg(src + f);
+      }
+    }
+  }
+  __syncwarp();
+  if (vis) {
+  const float* R = cam.R;
   // ---------------- colour: dL/dsh and the direction-dependent part of dL/dmean ----------------
   const float cpx = -(R[0] * cam.t[0] + R[3] * cam.t[1] + R[6] * cam.t[2]);
   const float cpy = -(R[1] * cam.t[0] + R[4] * cam.t[1] + R[7] * cam.t[2]);
@@ -56,10 +148,21 @@ __global__ void __launch_bounds__(128) preprocess_bwd_kernel(
   {
     // s_j = sum_k gcol_k sh[j][k];  dL/dsh[j][k] = Y_j gcol_k
     float sj[K], Y[K];
-    const float* shrow = sh + i * (3 * K);
+    {
+      float rowv[RK];
+      if (L::VEC) {
 #pragma unroll
-    for (int j = 0; j < K; j++)
-      sj[j] = gcol[0] * __ldg(shrow + 3 * j) + gcol[1] * __ldg(shrow + 3 * j + 1) + gcol[2] * __ldg(shrow + 3 * j + 2);
+        for (int j = 0; j < RK / 4; j++) {
+          const float4 v = *reinterpret_cast<const float4*>(myrow + 4 * j);
+          rowv[4 * j] = v.x; rowv[4 * j + 1] = v.y; rowv[4 * j + 2] = v.z; rowv[4 * j + 3] = v.w;
+        }
+      } else {
+#pragma unroll
+        for (int j = 0; j < RK; j++) rowv[j] = myrow[j];
+      }
+#pragma unroll
+      for (int j = 0; j < K; j++) sj[j] = gcol[0] * rowv[3 * j] + gcol[1] * rowv[3 * j + 1] + gcol[2] * rowv[3 * j + 2];
+    }
     const float xx = x * x, yy = y * y, zz = z * z;
     Y[0] = MG_SH_C0;
     float ddx = 0.f, ddy = 0.f, ddz = 0.f;  // dL/d(direction) treating Y_j as polynomials on R^3
@@ -101,23 +204,76 @@ __global__ void __launch_bounds__(128) preprocess_bwd_kernel(
     for (int j = 0; j < K; j++) {
       out[3 * j] = Y[j] * gcol[0]; out[3 * j + 1] = Y[j] * gcol[1]; out[3 * j + 2] = Y[j] * gcol[2];
     }
-    if ((3 * K) % 4 == 0) {
+    if (L::VEC) {
 #pragma unroll
-      for (int j = 0; j < 3 * K / 4; j++)
-        reinterpret_cast<float4*>(gsh)[j] = make_float4(out[4 * j], out[4 * j + 1], out[4 * j + 2], out[4 * j + 3]);
+      for (int j = 0; j < RK / 4; j++)
+        *reinterpret_cast<float4*>(myrow + 4 * j) = make_float4(out[4 * j], out[4 * j + 1], out[4 * j + 2], out[4 * j + 3]);
     } else {
 #pragma unroll
-      for (int j = 0; j < 3 * K; j++) gsh[j] = out[j];
+      for (int j = 0; j < RK; j++) myrow[j] = out[j];
     }
   }
 
-  // ---------------- geometry, in fp64 ----------------
+    dL_dmeans[3 * i] = dmx; dL_dmeans[3 * i + 1] = dmy; dL_dmeans[3 * i + 2] = dmz;
+  } else if (i < N) {
+    dL_dmeans[3 * i] = dL_dmeans[3 * i + 1] = dL_dmeans[3 * i + 2] = 0.f;
+  }
+  __syncwarp();
+  // coalesced store of dL/dsh: rows of visible Gaussians from shared memory, zeros for the others
+  if (nrows > 0) {
+    if (L::VEC) {
+      float4* dst = reinterpret_cast<float4*>(dL_dsh + g0 * RK);
+#pragma unroll
+      for (int k = 0; k < RK / 4; k++) {
+        const int f = k * 32 + lane, g = f / (RK / 4), c = f % (RK / 4);
+        if (g < nrows) {
+          float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+          if ((vmask >> g) & 1u) v = *reinterpret_cast<const float4*>(wrow + g * STRIDE + 4 * c);
+          dst[f] = v;
+        }
+      }
+    } else {
+      float* dst = dL_dsh + g0 * RK;
+#pragma unroll
+      for (int k = 0; k < RK; k++) {
+        const int f = k * 32 + lane, g = f / RK, c = f % RK;
+        if (g < nrows) dst[f] = ((vmask >> g) & 1u) ? wrow[g * STRIDE + c] : 0.f;
+      }
+    }
+  }
+}
+
+
+// Kernel 2 of 2: geometry.  Adds its part to dL_dmeans (written by kernel 1) and writes the other gradients.
+__global__ void __launch_bounds__(PB_THREADS, PB_MINB) preprocess_bwd_geo_kernel(
+    mg_camera cam, int64_t N, const float* __restrict__ means, const float* __restrict__ log_scales,
+    const float* __restrict__ quats, const float* __restrict__ opacity_logits, const int32_t* __restrict__ radii,
+    const float2* __restrict__ dL_dmeans2d, const float* __restrict__ dL_dconic, const float* __restrict__ dL_dopacity,
+    float* __restrict__ dL_dmeans, float* __restrict__ dL_dlog_scales, float4* __restrict__ dL_dquats,
+    float* __restrict__ dL_dopacity_logits) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  if (radii[i] <= 0) {  // culled: exact zeros everywhere (dL_dmeans was zeroed by kernel 1)
+    dL_dlog_scales[3 * i] = dL_dlog_scales[3 * i + 1] = dL_dlog_scales[3 * i + 2] = 0.f;
+    dL_dquats[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    dL_dopacity_logits[i] = 0.f;
+    return;
+  }
+  const float px = means[3 * i], py = means[3 * i + 1], pz = means[3 * i + 2];
+  const float4 q = __ldg(reinterpret_cast<const float4*>(quats) + i);
+  const double s0 = exp((double)log_scales[3 * i]), s1 = exp((double)log_scales[3 * i + 1]), s2 = exp((double)log_scales[3 * i + 2]);
+  const float o = 1.f / (1.f + expf(-opacity_logits[i]));
+  const float2 gm = dL_dmeans2d[i];
+  const float gA = dL_dconic[3 * i], gB = dL_dconic[3 * i + 1], gC = dL_dconic[3 * i + 2];
+  const float dmx = dL_dmeans[3 * i], dmy = dL_dmeans[3 * i + 1], dmz = dL_dmeans[3 * i + 2];  // colour part
+
+  // ---------------- geometry: forward chain and dL/dconic -> dL/dU in fp64 ----------------
   // dL/dconic is a sum of q d d^T over pixels; mapping it back through conic = Sigma2D^-1 contracts it
   // with vectors (A,B).d that are small for d along the major axis of an elongated splat, so the three
-  // products cancel to ~(k2/k1)^2 of their size.  fp32 loses up to 1e-3 of dL/dlog_scale there; this
-  // kernel is HBM-bound and ~300 fp64 flops per Gaussian are free, so the geometry chain runs in fp64
-  // on the fp32 inputs and is rounded once at the end.
-  typedef double G;
+  // products cancel to ~(k2/k1)^2 of their size.  fp32 loses up to 1e-3 of dL/dlog_scale there, so the
+  // forward chain up to det and the step conic -> covariance -> U run in fp64 on the fp32 inputs
+  // (~200 fp64 flops per Gaussian); the rest of the reverse pass is fp32.
+  typedef PB_G G;
   G Rd[9], td[3];
 #pragma unroll
   for (int j = 0; j < 9; j++) Rd[j] = (G)cam.R[j];
@@ -164,50 +320,15 @@ __global__ void __launch_bounds__(128) preprocess_bwd_kernel(
   // a = U0.U0, b = U0.U1, c = U1.U1
   const G dU00 = (G)2. * da * U00 + db * U10, dU01 = (G)2. * da * U01 + db * U11, dU02 = (G)2. * da * U02 + db * U12;
   const G dU10 = (G)2. * dc * U10 + db * U00, dU11 = (G)2. * dc * U11 + db * U01, dU12 = (G)2. * dc * U12 + db * U02;
-  // U = T M:  dT = dU M^T,  dM = T^T dU
-  const G dT00 = dU00 * M00 + dU01 * M01 + dU02 * M02, dT01 = dU00 * M10 + dU01 * M11 + dU02 * M12, dT02 = dU00 * M20 + dU01 * M21 + dU02 * M22;
-  const G dT10 = dU10 * M00 + dU11 * M01 + dU12 * M02, dT11 = dU10 * M10 + dU11 * M11 + dU12 * M12, dT12 = dU10 * M20 + dU11 * M21 + dU12 * M22;
-  const G dM00 = T00 * dU00 + T10 * dU10, dM01 = T00 * dU01 + T10 * dU11, dM02 = T00 * dU02 + T10 * dU12;
-  const G dM10 = T01 * dU00 + T11 * dU10, dM11 = T01 * dU01 + T11 * dU11, dM12 = T01 * dU02 + T11 * dU12;
-  const G dM20 = T02 * dU00 + T12 * dU10, dM21 = T02 * dU01 + T12 * dU11, dM22 = T02 * dU02 + T12 * dU12;
-  // M = Rot diag(s)
-  const G ds0 = dM00 * r00 + dM10 * r10 + dM20 * r20;
-  const G ds1 = dM01 * r01 + dM11 * r11 + dM21 * r21;
-  const G ds2 = dM02 * r02 + dM12 * r12 + dM22 * r22;
-  dL_dlog_scales[3 * i] = (float)(ds0 * s0);
-  dL_dlog_scales[3 * i + 1] = (float)(ds1 * s1);
-  dL_dlog_scales[3 * i + 2] = (float)(ds2 * s2);
-  const G dr00 = dM00 * s0, dr01 = dM01 * s1, dr02 = dM02 * s2;
-  const G dr10 = dM10 * s0, dr11 = dM11 * s1, dr12 = dM12 * s2;
-  const G dr20 = dM20 * s0, dr21 = dM21 * s1, dr22 = dM22 * s2;
-  // Rot(unit quaternion)
-  const G dqw = (G)2. * (-qz * dr01 + qy * dr02 + qz * dr10 - qx * dr12 - qy * dr20 + qx * dr21);
-  const G dqx = (G)2. * (qy * dr01 + qz * dr02 + qy * dr10 - (G)2. * qx * dr11 - qw * dr12 + qz * dr20 + qw * dr21 - (G)2. * qx * dr22);
-  const G dqy = (G)2. * (-(G)2. * qy * dr00 + qx * dr01 + qw * dr02 + qx * dr10 + qz * dr12 - qw * dr20 + qz * dr21 - (G)2. * qy * dr22);
-  const G dqz = (G)2. * (-(G)2. * qz * dr00 - qw * dr01 + qx * dr02 + qw * dr10 - (G)2. * qz * dr11 + qy * dr12 + qx * dr20 + qy * dr21);
-  // through q / |q|
-  const G qdot = qw * dqw + qx * dqx + qy * dqy + qz * dqz;
-  dL_dquats[i] = make_float4((float)((dqw - qw * qdot) * qinv), (float)((dqx - qx * qdot) * qinv), (float)((dqy - qy * qdot) * qinv), (float)((dqz - qz * qdot) * qinv));
-  // T = J W
-  const G dJ00 = dT00 * Rd[0] + dT01 * Rd[1] + dT02 * Rd[2];
-  const G dJ02 = dT00 * Rd[6] + dT01 * Rd[7] + dT02 * Rd[8];
-  const G dJ11 = dT10 * Rd[3] + dT11 * Rd[4] + dT12 * Rd[5];
-  const G dJ12 = dT10 * Rd[6] + dT11 * Rd[7] + dT12 * Rd[8];
-  // J(t) and the projected centre
-  const G iz2 = iz * iz;
-  G dtx = gm.x * fxd * iz, dty = gm.y * fyd * iz;
-  G dtz = -(dJ00 * fxd + dJ11 * fyd) * iz2 - ((G)gm.x * fxd * tx + (G)gm.y * fyd * ty) * iz2;
-  if (xcl) dtz += dJ02 * fxd * xz * iz2;  // J02 = -fx L / z with L = +-limx
-  else { dtx += -dJ02 * fxd * iz2; dtz += dJ02 * (G)2. * fxd * tx * iz2 * iz; }
-  if (ycl) dtz += dJ12 * fyd * yz * iz2;
-  else { dty += -dJ12 * fyd * iz2; dtz += dJ12 * (G)2. * fyd * ty * iz2 * iz; }
-  // t = R p + t_cam
-  const G dmx_g = Rd[0] * dtx + Rd[3] * dty + Rd[6] * dtz;
-  const G dmy_g = Rd[1] * dtx + Rd[4] * dty + Rd[7] * dtz;
-  const G dmz_g = Rd[2] * dtx + Rd[5] * dty + Rd[8] * dtz;
-  dL_dmeans[3 * i] = (float)((G)dmx + dmx_g);
-  dL_dmeans[3 * i + 1] = (float)((G)dmy + dmy_g);
-  dL_dmeans[3 * i + 2] = (float)((G)dmz + dmz_g);
+  // from dL/dU on: well-conditioned, fp32 (see geometry_tail)
+  typedef PB_H H;
+  H Rh[9];
+#pragma unroll
+  for (int j = 0; j < 9; j++) Rh[j] = (H)cam.R[j];
+  const GeoGrads gg = geometry_tail<H>(Rh, xcl, ycl, (H)dU00, (H)dU01, (H)dU02, (H)dU10, (H)dU11, (H)dU12, (H)M00, (H)M01, (H)M02, (H)M10, (H)M11, (H)M12, (H)M20, (H)M21, (H)M22, (H)T00, (H)T01, (H)T02, (H)T10, (H)T11, (H)T12, (H)r00, (H)r01, (H)r02, (H)r10, (H)r11, (H)r12, (H)r20, (H)r21, (H)r22, (H)s0, (H)s1, (H)s2, (H)qw, (H)qx, (H)qy, (H)qz, (H)qinv, (H)fxd, (H)fyd, (H)iz, (H)tx, (H)ty, (H)xz, (H)yz, (H)gm.x, (H)gm.y, (H)dmx, (H)dmy, (H)dmz);
+  dL_dlog_scales[3 * i] = gg.dls[0]; dL_dlog_scales[3 * i + 1] = gg.dls[1]; dL_dlog_scales[3 * i + 2] = gg.dls[2];
+  dL_dquats[i] = gg.dq;
+  dL_dmeans[3 * i] = gg.dm[0]; dL_dmeans[3 * i + 1] = gg.dm[1]; dL_dmeans[3 * i + 2] = gg.dm[2];
   dL_dopacity_logits[i] = dL_dopacity[i] * o * ((G)1. - o);
 }
 
@@ -225,14 +346,11 @@ extern "C" int mg_preprocess_bwd(const mg_camera* cam, int64_t N, const float* m
   MG_REQUIRE(means && log_scales && quats && opacity_logits && sh && radii && clamped, "null input array");
   MG_REQUIRE(dL_dmeans2d && dL_dconic && dL_dopacity && dL_drgb, "null upstream gradient");
   MG_REQUIRE(dL_dmeans && dL_dlog_scales && dL_dquats && dL_dopacity_logits && dL_dsh, "null output gradient");
-  const int threads = 128;
+  const int threads = PB_THREADS;
   const unsigned blocks = (unsigned)((N + threads - 1) / threads);
   cudaStream_t st = (cudaStream_t)stream;
-#define MG_LAUNCH(D)                                                                                              \
-  preprocess_bwd_kernel<D><<<blocks, threads, 0, st>>>(*cam, N, means, log_scales, quats, opacity_logits, sh,     \
-                                                       radii, clamped, (const float2*)dL_dmeans2d, dL_dconic,     \
-                                                       dL_dopacity, dL_drgb, dL_dmeans, dL_dlog_scales,           \
-                                                       (float4*)dL_dquats, dL_dopacity_logits, dL_dsh)
+#define MG_LAUNCH(D)                                                                                            \
+  preprocess_bwd_sh_kernel<D><<<blocks, threads, 0, st>>>(*cam, N, means, sh, radii, clamped, dL_drgb, dL_dmeans, dL_dsh)
   switch (cam->sh_degree) {
     case 0: MG_LAUNCH(0); break;
     case 1: MG_LAUNCH(1); break;
@@ -240,6 +358,10 @@ extern "C" int mg_preprocess_bwd(const mg_camera* cam, int64_t N, const float* m
     default: MG_LAUNCH(3); break;
   }
 #undef MG_LAUNCH
+  MG_CHECK_LAUNCH();
+  preprocess_bwd_geo_kernel<<<blocks, threads, 0, st>>>(*cam, N, means, log_scales, quats, opacity_logits, radii,
+                                                        (const float2*)dL_dmeans2d, dL_dconic, dL_dopacity, dL_dmeans,
+                                                        dL_dlog_scales, (float4*)dL_dquats, dL_dopacity_logits);
   MG_CHECK_LAUNCH();
   return MG_OK;
 }
