@@ -87,22 +87,29 @@ int mg_preprocess(const mg_camera* cam, int64_t N, const float* means, const flo
  * 64-bit key (tile_id << 32 | fp32 bits of depth), ties by Gaussian index, tile_id = ty * gw + tx:
  *   sorted_ids[R]       Gaussian index of each sorted key
  *   tile_ranges[gw*gh][2] = [start, end) of each tile in sorted_ids (start == end for an empty tile)
+ *   tile_order[gw*gh] (may be NULL): a scheduling hint for the two render calls -- a permutation of the tile
+ *                       ids in which the length class of the tile lists never increases (class(0) = 0,
+ *                       class(n) = 1 + 8 floor(log2 n) + the next 3 bits of n), so that a grid launched in this
+ *                       order starts its longest tiles first.  The order within a class is unspecified.
  *   R_out_host (may be NULL): the true R, written asynchronously.
  * R must be < 2^32.  If R > R_capacity nothing is written to sorted_ids, every tile range is set to
  * [0, 0) and *R_out_host (> R_capacity) tells the caller to retry with larger buffers.
  * workspace: at least mg_workspace_bytes(N, W, H, R_capacity) bytes, 256-byte aligned. */
 int mg_bin_sort(const mg_camera* cam, int64_t N, const float* depths, const int32_t* rects,
                 const uint32_t* tiles_touched, uint64_t R_capacity, void* workspace, size_t workspace_bytes,
-                uint32_t* sorted_ids, uint32_t* tile_ranges, uint64_t* R_out_host, void* stream);
+                uint32_t* sorted_ids, uint32_t* tile_ranges, uint32_t* tile_order, uint64_t* R_out_host,
+                void* stream);
 
 /* Step a7 (Eq. 3-4; Eq. 9-10).  Per pixel, front to back over its tile's
  * list: alpha = min(0.99, o G); skip if power > 0 or alpha < 1/255 (mask NOT consulted, reading 2);
  * a = M alpha; T' = T (1 - a); stop if T' < 1e-4 (this entry is not blended, reading 3-4);
  * C += a T c; T = T'.  Then image = C + T c_bg.
  *   image[3][H][W]; final_T[H][W] = T_{N+1}; n_contrib[H][W] = 1-based list position of the last entry
- *   that was blended, masked or not (0 if none; reading 5). */
+ *   that was blended, masked or not (0 if none; reading 5).
+ *   tile_order (may be NULL = row-major): the order in which tiles are scheduled (mg_bin_sort's hint); it has
+ *   no effect on any output. */
 int mg_render_fwd(const mg_camera* cam, const uint32_t* sorted_ids, const uint32_t* tile_ranges,
-                  const float* means2d, const float* conic_opacity, const float* rgb, const float* masks,
+                  const uint32_t* tile_order, const float* means2d, const float* conic_opacity, const float* rgb, const float* masks,
                   float* image, float* final_T, uint32_t* n_contrib, void* stream);
 
 /* Step a8 (Eq. 11, 13-18).  Per pixel, from its last contributor back to the front:
@@ -110,9 +117,10 @@ int mg_render_fwd(const mg_camera* cam, const uint32_t* sorted_ids, const uint32
  * term); dL/dalpha_i = M_i * (same bracket); chain to colour, opacity (w.r.t. the activated o), conic and
  * projected centre (pixels).  Zero gradient to (o, conic, centre) where the 0.99 clamp is active
  * (reading 6).  A masked Gaussian (M = 0) gets dL/dM only (Fig. 1).
- * Sums over pixels use fp32 atomics: results vary in the last bits from run to run. */
+ * Sums over pixels use fp32 atomics: results vary in the last bits from run to run.
+ * tile_order: as for mg_render_fwd. */
 int mg_render_bwd(const mg_camera* cam, int64_t N, const uint32_t* sorted_ids, const uint32_t* tile_ranges,
-                  const float* means2d, const float* conic_opacity, const float* rgb, const float* masks,
+                  const uint32_t* tile_order, const float* means2d, const float* conic_opacity, const float* rgb, const float* masks,
                   const float* final_T, const uint32_t* n_contrib, const float* dL_dimage, float* dL_dmeans2d,
                   float* dL_dconic, float* dL_dopacity, float* dL_drgb, float* dL_dmask, void* stream);
 

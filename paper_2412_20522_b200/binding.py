@@ -109,25 +109,26 @@ def mg_preprocess(cam: mg_camera, means, log_scales, quats, opacity_logits, sh, 
 
 
 def mg_bin_sort(cam: mg_camera, depths, rects, tiles_touched, R_capacity, workspace, sorted_ids, tile_ranges,
-                R_out_host=None):
+                R_out_host=None, tile_order=None):
     N = depths.shape[0]
     _check(lib().mg_bin_sort(C.byref(cam), C.c_int64(N), _ptr(depths, F32), _ptr(rects, I32), _ptr(tiles_touched, I32),
                              C.c_uint64(int(R_capacity)), _ptr(workspace, U8), C.c_size_t(workspace.numel()),
-                             _ptr(sorted_ids, I32), _ptr(tile_ranges, I32), _ptr(R_out_host, torch.int64, "cpu"),
-                             _stream()))
+                             _ptr(sorted_ids, I32), _ptr(tile_ranges, I32), _ptr(tile_order, I32),
+                             _ptr(R_out_host, torch.int64, "cpu"), _stream()))
 
 
 def mg_render_fwd(cam: mg_camera, sorted_ids, tile_ranges, means2d, conic_opacity, rgb, masks, image, final_T,
-                  n_contrib):
-    _check(lib().mg_render_fwd(C.byref(cam), _ptr(sorted_ids, I32), _ptr(tile_ranges, I32), _ptr(means2d, F32),
+                  n_contrib, tile_order=None):
+    _check(lib().mg_render_fwd(C.byref(cam), _ptr(sorted_ids, I32), _ptr(tile_ranges, I32), _ptr(tile_order, I32),
+                               _ptr(means2d, F32),
                                _ptr(conic_opacity, F32), _ptr(rgb, F32), _ptr(masks, F32), _ptr(image, F32),
                                _ptr(final_T, F32), _ptr(n_contrib, I32), _stream()))
 
 
 def mg_render_bwd(cam: mg_camera, N, sorted_ids, tile_ranges, means2d, conic_opacity, rgb, masks, final_T, n_contrib,
-                  dL_dimage, dL_dmeans2d, dL_dconic, dL_dopacity, dL_drgb, dL_dmask):
+                  dL_dimage, dL_dmeans2d, dL_dconic, dL_dopacity, dL_drgb, dL_dmask, tile_order=None):
     _check(lib().mg_render_bwd(C.byref(cam), C.c_int64(N), _ptr(sorted_ids, I32), _ptr(tile_ranges, I32),
-                               _ptr(means2d, F32), _ptr(conic_opacity, F32), _ptr(rgb, F32), _ptr(masks, F32),
+                               _ptr(tile_order, I32), _ptr(means2d, F32), _ptr(conic_opacity, F32), _ptr(rgb, F32), _ptr(masks, F32),
                                _ptr(final_T, F32), _ptr(n_contrib, I32), _ptr(dL_dimage, F32), _ptr(dL_dmeans2d, F32),
                                _ptr(dL_dconic, F32), _ptr(dL_dopacity, F32), _ptr(dL_drgb, F32), _ptr(dL_dmask, F32),
                                _stream()))
@@ -164,6 +165,7 @@ class Frame:
         self.radii, self.rects, self.tiles_touched = e(N, dt=I32), e(N, 4, dt=I32), e(N, dt=I32)
         self.clamped = e(N, dt=U8)
         self.tile_ranges = e(gw * gh, 2, dt=I32)
+        self.tile_order = e(gw * gh, dt=I32)  # scheduling hint: longest tile lists first
         self.image, self.final_T, self.n_contrib = e(3, H, W), e(H, W), e(H, W, dt=I32)
         self.dL_dmeans2d, self.dL_dconic, self.dL_dopacity = e(N, 2), e(N, 3), e(N)
         self.dL_drgb, self.dL_dmask = e(N, 3), e(N)
@@ -190,16 +192,16 @@ class Frame:
 
     def bin_sort(self):
         mg_bin_sort(self.cam, self.depths, self.rects, self.tiles_touched, self.R_capacity, self.workspace,
-                    self.sorted_ids, self.tile_ranges, self.R_host[1:2])
+                    self.sorted_ids, self.tile_ranges, self.R_host[1:2], self.tile_order)
 
     def render_fwd(self, masks):
         mg_render_fwd(self.cam, self.sorted_ids, self.tile_ranges, self.means2d, self.conic_opacity, self.rgb, masks,
-                      self.image, self.final_T, self.n_contrib)
+                      self.image, self.final_T, self.n_contrib, self.tile_order)
 
     def render_bwd(self, masks, dL_dimage):
         mg_render_bwd(self.cam, self.N, self.sorted_ids, self.tile_ranges, self.means2d, self.conic_opacity, self.rgb,
                       masks, self.final_T, self.n_contrib, dL_dimage, self.dL_dmeans2d, self.dL_dconic,
-                      self.dL_dopacity, self.dL_drgb, self.dL_dmask)
+                      self.dL_dopacity, self.dL_drgb, self.dL_dmask, self.tile_order)
 
     def preprocess_bwd(self, g):
         mg_preprocess_bwd(self.cam, g["means"], g["log_scales"], g["quats"], g["opacity_logits"], g["sh"], self.radii,

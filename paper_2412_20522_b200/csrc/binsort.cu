@@ -42,6 +42,16 @@ constexpr int SCAN_THREADS = 1024;
 constexpr int SCAN_ITEMS = 4;
 constexpr int SCAN_BLK = SCAN_THREADS * SCAN_ITEMS;
 
+constexpr int TO_CLASSES = 257;  // list-length classes of the scheduling hint tile_order
+
+// class(0) = 0, class(n) = 1 + 8 floor(log2 n) + the next 3 bits of n: monotone in n, integer-only.
+__device__ __forceinline__ uint32_t length_class(uint32_t n) {
+  if (n == 0) return 0u;
+  const int msb = 31 - __clz(n);
+  const uint32_t frac = msb >= 3 ? (n >> (msb - 3)) & 7u : (n << (3 - msb)) & 7u;
+  return 1u + 8u * (uint32_t)msb + frac;
+}
+
 struct SortCtl {            // lives in the workspace; zeroed at the start of every call
   unsigned long long R;     // true number of duplicated keys = sum of tiles_touched
   uint32_t nvis;            // Gaussians with tiles_touched > 0
@@ -49,6 +59,8 @@ struct SortCtl {            // lives in the workspace; zeroed at the start of ev
   uint32_t n_chunks_c;      // chunks of the column expansion (sum over rows of ceil(records / XP_CHUNK))
   uint32_t n_table_c;       // gw * n_chunks_c
   uint32_t pad[2];
+  uint32_t class_count[TO_CLASSES];   // tiles per list-length class (tile_order)
+  uint32_t class_cursor[TO_CLASSES];  // tiles of the class already placed
 };
 
 // One stable radix pass on 8 bits at `shift`.  kCount: write the per-block digit histogram to
@@ -431,7 +443,7 @@ __global__ void __launch_bounds__(32 * XP_MAX_WARPS) col_expand_kernel(
 // records has no table entries and all its tiles start (and end) where the next row's first tile starts.
 __global__ void __launch_bounds__(256) tile_ranges_kernel(const uint32_t* __restrict__ table_c,
                                                           const uint32_t* __restrict__ chunk_base,
-                                                          const SortCtl* __restrict__ ctl, int gw, int gh,
+                                                          SortCtl* __restrict__ ctl, int gw, int gh,
                                                           uint32_t* __restrict__ tile_ranges) {
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
   const int ntiles = gw * gh;
@@ -439,6 +451,7 @@ __global__ void __launch_bounds__(256) tile_ranges_kernel(const uint32_t* __rest
   if (ctl->overflow) {
     tile_ranges[2 * t] = 0;
     tile_ranges[2 * t + 1] = 0;
+    atomicAdd(&ctl->class_count[0], 1u);
     return;
   }
   uint32_t se[2];
@@ -456,6 +469,23 @@ __global__ void __launch_bounds__(256) tile_ranges_kernel(const uint32_t* __rest
   }
   tile_ranges[2 * t] = se[0];
   tile_ranges[2 * t + 1] = se[1];
+  atomicAdd(&ctl->class_count[length_class(se[1] - se[0])], 1u);
+}
+
+// Scheduling hint: tiles in order of non-increasing list-length class (the order within a class is whatever
+// the atomics give; it affects scheduling only).  Every block rebuilds the 257 class bases in shared memory.
+__global__ void __launch_bounds__(256) tile_order_kernel(const uint32_t* __restrict__ tile_ranges, SortCtl* __restrict__ ctl,
+                                                         int ntiles, uint32_t* __restrict__ tile_order) {
+  __shared__ uint32_t base[TO_CLASSES];
+  if (threadIdx.x == 0) {
+    uint32_t run = 0;
+    for (int c = TO_CLASSES - 1; c >= 0; c--) { base[c] = run; run += ctl->class_count[c]; }
+  }
+  __syncthreads();
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= ntiles) return;
+  const uint32_t c = length_class(tile_ranges[2 * t + 1] - tile_ranges[2 * t]);
+  tile_order[base[c] + atomicAdd(&ctl->class_cursor[c], 1u)] = (uint32_t)t;
 }
 
 struct Layout {
@@ -529,7 +559,8 @@ extern "C" size_t mg_workspace_bytes(int64_t N, int32_t width, int32_t height, u
 
 extern "C" int mg_bin_sort(const mg_camera* cam, int64_t N, const float* depths, const int32_t* rects,
                            const uint32_t* tiles_touched, uint64_t R_capacity, void* workspace, size_t workspace_bytes,
-                           uint32_t* sorted_ids, uint32_t* tile_ranges, uint64_t* R_out_host, void* stream) {
+                           uint32_t* sorted_ids, uint32_t* tile_ranges, uint32_t* tile_order, uint64_t* R_out_host,
+                           void* stream) {
   if (int rc = mg_check_camera(cam)) return rc;
   MG_REQUIRE(N >= 0 && N < (int64_t)1 << 31, "N must be in [0, 2^31)");
   MG_REQUIRE(R_capacity < (1ull << 32), "R_capacity must be < 2^32");
@@ -558,6 +589,10 @@ extern "C" int mg_bin_sort(const mg_camera* cam, int64_t N, const float* depths,
   MG_CHECK_CUDA(cudaMemsetAsync(ctl, 0, sizeof(SortCtl), st));
   if (N == 0) {
     MG_CHECK_CUDA(cudaMemsetAsync(tile_ranges, 0, sizeof(uint32_t) * 2 * (size_t)gw * gh, st));
+    if (tile_order) {
+      tile_order_kernel<<<(gw * gh + 255) / 256, 256, 0, st>>>(tile_ranges, ctl, gw * gh, tile_order);
+      MG_CHECK_LAUNCH();
+    }
     if (R_out_host) MG_CHECK_CUDA(cudaMemcpyAsync(R_out_host, &ctl->R, sizeof(uint64_t), cudaMemcpyDeviceToHost, st));
     return MG_OK;
   }
@@ -607,6 +642,7 @@ extern "C" int mg_bin_sort(const mg_camera* cam, int64_t N, const float* depths,
     if (int rc = scan_table(table_c, 0, &ctl->n_table_c, tc_max, sums, st)) return rc;
     col_expand_kernel<false><<<grid, 32 * wpb, smem, st>>>(row_rec, row_start, chunk_base, ctl, gw, gh, wpb, table_c, sorted_ids);
     tile_ranges_kernel<<<(gw * gh + 255) / 256, 256, 0, st>>>(table_c, chunk_base, ctl, gw, gh, tile_ranges);
+    if (tile_order) tile_order_kernel<<<(gw * gh + 255) / 256, 256, 0, st>>>(tile_ranges, ctl, gw * gh, tile_order);
     MG_CHECK_LAUNCH();
   }
   if (R_out_host) MG_CHECK_CUDA(cudaMemcpyAsync(R_out_host, &ctl->R, sizeof(uint64_t), cudaMemcpyDeviceToHost, st));

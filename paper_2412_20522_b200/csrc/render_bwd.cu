@@ -83,14 +83,14 @@ __device__ __forceinline__ float warp_sum(float v) {
 
 __global__ void __launch_bounds__(RN_THREADS, RN_BWD_MINB) render_bwd_kernel(
     int W, int H, int gw, float bg0, float bg1, float bg2, const uint32_t* __restrict__ sorted_ids,
-    const uint2* __restrict__ tile_ranges, const float2* __restrict__ means2d,
-    const float4* __restrict__ conic_opacity, const float* __restrict__ rgb, const float* __restrict__ masks,
-    const float* __restrict__ final_T, const uint32_t* __restrict__ n_contrib, const float* __restrict__ dL_dimage,
+    const uint2* __restrict__ tile_ranges, const uint32_t* __restrict__ tile_order,
+    const float2* __restrict__ means2d, const float4* __restrict__ conic_opacity, const float* __restrict__ rgb,
+    const float* __restrict__ masks, const float* __restrict__ final_T, const uint32_t* __restrict__ n_contrib, const float* __restrict__ dL_dimage,
     BwdTargets tg) {
   __shared__ RnRecord buf_all[RN_WARPS][32];
   __shared__ RnStage stage_all[RN_WARPS];
   __shared__ uint32_t ids_all[RN_WARPS][32];
-  const int tile = blockIdx.x;
+  const int tile = tile_order ? (int)tile_order[blockIdx.x] : (int)blockIdx.x;  // longest lists first
   const int tx = tile % gw, ty = tile / gw;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   RnRecord* buf = buf_all[warp];
@@ -261,7 +261,7 @@ __global__ void __launch_bounds__(RN_THREADS, RN_BWD_MINB) render_bwd_kernel(
 }  // namespace
 
 extern "C" int mg_render_bwd(const mg_camera* cam, int64_t N, const uint32_t* sorted_ids, const uint32_t* tile_ranges,
-                             const float* means2d, const float* conic_opacity, const float* rgb, const float* masks,
+                             const uint32_t* tile_order, const float* means2d, const float* conic_opacity, const float* rgb, const float* masks,
                              const float* final_T, const uint32_t* n_contrib, const float* dL_dimage,
                              float* dL_dmeans2d, float* dL_dconic, float* dL_dopacity, float* dL_drgb, float* dL_dmask,
                              void* stream) {
@@ -285,7 +285,7 @@ extern "C" int mg_render_bwd(const mg_camera* cam, int64_t N, const uint32_t* so
   for (int s = 0; s < 10; s++) { tg.base[s] = bases[s]; tg.stride[s] = strides[s]; tg.offset[s] = offsets[s]; }
   const int gw = mg_grid_w(cam), gh = mg_grid_h(cam);
   render_bwd_kernel<<<gw * gh, RN_THREADS, 0, st>>>(cam->width, cam->height, gw, cam->bg[0], cam->bg[1], cam->bg[2],
-                                                    sorted_ids, (const uint2*)tile_ranges, (const float2*)means2d,
+                                                    sorted_ids, (const uint2*)tile_ranges, tile_order, (const float2*)means2d,
                                                     (const float4*)conic_opacity, rgb, masks, final_T, n_contrib,
                                                     dL_dimage, tg);
   MG_CHECK_LAUNCH();

@@ -21,12 +21,12 @@ namespace {
 
 __global__ void __launch_bounds__(RN_THREADS, RN_FWD_MINB) render_fwd_kernel(
     int W, int H, int gw, float bg0, float bg1, float bg2, const uint32_t* __restrict__ sorted_ids,
-    const uint2* __restrict__ tile_ranges, const float2* __restrict__ means2d,
-    const float4* __restrict__ conic_opacity, const float* __restrict__ rgb, const float* __restrict__ masks,
-    float* __restrict__ image, float* __restrict__ final_T, uint32_t* __restrict__ n_contrib) {
+    const uint2* __restrict__ tile_ranges, const uint32_t* __restrict__ tile_order,
+    const float2* __restrict__ means2d, const float4* __restrict__ conic_opacity, const float* __restrict__ rgb,
+    const float* __restrict__ masks, float* __restrict__ image, float* __restrict__ final_T, uint32_t* __restrict__ n_contrib) {
   __shared__ RnRecord buf_all[RN_WARPS][32];
   __shared__ RnStage stage_all[RN_WARPS];
-  const int tile = blockIdx.x;
+  const int tile = tile_order ? (int)tile_order[blockIdx.x] : (int)blockIdx.x;  // longest lists first
   const int tx = tile % gw, ty = tile / gw;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   RnRecord* buf = buf_all[warp];
@@ -149,7 +149,7 @@ __global__ void __launch_bounds__(RN_THREADS, RN_FWD_MINB) render_fwd_kernel(
 }  // namespace
 
 extern "C" int mg_render_fwd(const mg_camera* cam, const uint32_t* sorted_ids, const uint32_t* tile_ranges,
-                             const float* means2d, const float* conic_opacity, const float* rgb, const float* masks,
+                             const uint32_t* tile_order, const float* means2d, const float* conic_opacity, const float* rgb, const float* masks,
                              float* image, float* final_T, uint32_t* n_contrib, void* stream) {
   if (int rc = mg_check_camera(cam)) return rc;
   MG_REQUIRE(tile_ranges && image && final_T && n_contrib, "null output or tile_ranges");
@@ -157,7 +157,7 @@ extern "C" int mg_render_fwd(const mg_camera* cam, const uint32_t* sorted_ids, c
   const int gw = mg_grid_w(cam), gh = mg_grid_h(cam);
   render_fwd_kernel<<<gw * gh, RN_THREADS, 0, (cudaStream_t)stream>>>(
       cam->width, cam->height, gw, cam->bg[0], cam->bg[1], cam->bg[2], sorted_ids, (const uint2*)tile_ranges,
-      (const float2*)means2d, (const float4*)conic_opacity, rgb, masks, image, final_T, n_contrib);
+      tile_order, (const float2*)means2d, (const float4*)conic_opacity, rgb, masks, image, final_T, n_contrib);
   MG_CHECK_LAUNCH();
   return MG_OK;
 }

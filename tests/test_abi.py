@@ -60,13 +60,13 @@ def test_invalid_arguments_are_rejected_without_a_gpu(lib):
 
     cam = binding.mg_camera()
     cam.width, cam.height, cam.fx, cam.fy, cam.sh_degree = 64, 64, 50.0, 50.0, 7
-    rc = lib.mg_render_fwd(C.byref(cam), *[C.c_void_p(0)] * 10)
+    rc = lib.mg_render_fwd(C.byref(cam), *[C.c_void_p(0)] * 11)
     assert rc == binding.MG_ERR_INVALID_ARG and b"sh_degree" in lib.mg_last_error_string()
     cam.sh_degree = 0
-    rc = lib.mg_render_fwd(C.byref(cam), *[C.c_void_p(0)] * 10)
+    rc = lib.mg_render_fwd(C.byref(cam), *[C.c_void_p(0)] * 11)
     assert rc == binding.MG_ERR_INVALID_ARG and b"null" in lib.mg_last_error_string()
     rc = lib.mg_bin_sort(C.byref(cam), C.c_int64(-5), *[C.c_void_p(0)] * 3, C.c_uint64(0), C.c_void_p(0), C.c_size_t(0),
-                         *[C.c_void_p(0)] * 4)
+                         *[C.c_void_p(0)] * 5)
     assert rc == binding.MG_ERR_INVALID_ARG
     rc = lib.mg_preprocess(None, C.c_int64(1), *[C.c_void_p(0)] * 15)
     assert rc == binding.MG_ERR_INVALID_ARG

@@ -229,3 +229,38 @@ def test_many_tiles_three_sort_passes(oracle):
     fr.forward(g, m)
     torch.cuda.synchronize()
     pu.check_bin_sort(fr, cam)
+
+
+def _length_class(n):
+    """include/mg.h: class(0) = 0, class(n) = 1 + 8 floor(log2 n) + the next 3 bits of n."""
+    n = np.asarray(n, np.int64)
+    msb = np.zeros_like(n)
+    nz = n > 0
+    msb[nz] = np.floor(np.log2(n[nz])).astype(np.int64)
+    msb[nz] -= (1 << msb[nz]) > n[nz]  # guard log2 rounding
+    msb[nz] += (1 << (msb[nz] + 1)) <= n[nz]
+    frac = np.where(msb >= 3, (n >> np.maximum(msb - 3, 0)) & 7, (n << np.maximum(3 - msb, 0)) & 7)
+    return np.where(nz, 1 + 8 * msb + frac, 0)
+
+
+def test_tile_order_is_a_permutation_with_longest_lists_first(run):
+    """mg_bin_sort's scheduling hint: a permutation of the tiles, list-length class never increasing."""
+    name, sc, fr = run
+    order = fr.tile_order.cpu().numpy().astype(np.int64)
+    ranges = fr.tile_ranges.cpu().numpy().astype(np.int64)
+    ntiles = ranges.shape[0]
+    assert sorted(order.tolist()) == list(range(ntiles))
+    cls = _length_class(ranges[order, 1] - ranges[order, 0])
+    assert (np.diff(cls) <= 0).all()
+
+
+def test_tile_order_does_not_change_the_image(run):
+    """The render calls give bit-identical per-pixel outputs with the hint and without it (row-major)."""
+    name, sc, fr = run
+    g, m = mg.upload(sc)
+    fr.render_fwd(m)
+    img, fT, nc = fr.image.clone(), fr.final_T.clone(), fr.n_contrib.clone()
+    mg.mg_render_fwd(fr.cam, fr.sorted_ids, fr.tile_ranges, fr.means2d, fr.conic_opacity, fr.rgb, m, fr.image,
+                     fr.final_T, fr.n_contrib, tile_order=None)
+    torch.cuda.synchronize()
+    assert torch.equal(img, fr.image) and torch.equal(fT, fr.final_T) and torch.equal(nc, fr.n_contrib)
