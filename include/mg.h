@@ -104,8 +104,11 @@ int mg_bin_sort(const mg_camera* cam, int64_t N, const float* depths, const int3
  * list: alpha = min(0.99, o G); skip if power > 0 or alpha < 1/255 (mask NOT consulted, reading 2);
  * a = M alpha; T' = T (1 - a); stop if T' < 1e-4 (this entry is not blended, reading 3-4);
  * C += a T c; T = T'.  Then image = C + T c_bg.
- *   image[3][H][W]; final_T[H][W] = T_{N+1}; n_contrib[H][W] = 1-based list position of the last entry
- *   that was blended, masked or not (0 if none; reading 5).
+ *   image[3][H][W]; final_T[H][W] = T_{N+1}; n_contrib[H][W] = the number of list entries the pixel
+ *   consumed: the entries in front of the one that stopped it, or the length of the tile's list if nothing
+ *   stopped it (reading 5).  It bounds the reverse traversal: every entry that contributed to the pixel,
+ *   masked or not, lies at a 1-based position <= n_contrib, and no entry at or behind the stop does.  The
+ *   forward pass therefore never has to look at an entry with M = 0.
  *   tile_order (may be NULL = row-major): the order in which tiles are scheduled (mg_bin_sort's hint); it has
  *   no effect on any output. */
 int mg_render_fwd(const mg_camera* cam, const uint32_t* sorted_ids, const uint32_t* tile_ranges,

@@ -305,7 +305,10 @@ int orc_bin_sort(const Cam* cam, int64_t N, const float* depths, const int32_t* 
 }
 
 // Walk one pixel's list front to back (O10).  Fills `pass` (entries that passed the alpha
-// filter and were blended) and returns the final transmittance.  `margin` receives the smallest
+// filter and were blended) and returns the final transmittance.  `last` receives the number of list
+// entries the pixel consumed: the entries in front of the one that stopped it, or the whole list if
+// nothing stopped it (reading 5).  Every entry the reverse traversal must visit lies at a
+// position <= last, and no entry at or behind the stop does.  `margin` receives the smallest
 // relative distance of any decision from its flip point; `hash` a signature of all decisions.
 static double walk_pixel(double px, double py, const uint32_t* ids, uint32_t n, const double* means2d,
                          const double* conic_opacity, const float* masks, std::vector<Passing>* pass, uint32_t* last,
@@ -313,7 +316,7 @@ static double walk_pixel(double px, double py, const uint32_t* ids, uint32_t n, 
   double T = 1.0, mg = 1e30, mgc = 1e30;
   uint64_t h = 1469598103934665603ull;
   auto mix = [&](uint64_t v) { h = (h ^ v) * 1099511628211ull; };
-  *last = 0;
+  *last = n;
   for (uint32_t k = 0; k < n; k++) {
     const uint32_t id = ids[k];
     (*n_eval)++;
@@ -331,10 +334,9 @@ static double walk_pixel(double px, double py, const uint32_t* ids, uint32_t n, 
     const double a = (double)masks[id] * alpha;  // Eq. 4: T_{i+1} = (1 - M_i alpha_i) T_i
     const double Tn = T * (1.0 - a);
     mg = std::min(mg, std::fabs(Tn - T_MIN) / T_MIN);
-    if (Tn < T_MIN) { mix(id * 4ull + 2); break; }  // not blended, not counted
+    if (Tn < T_MIN) { mix(id * 4ull + 2); *last = k; break; }  // not blended, not counted: k entries consumed
     mix(id * 4ull + 3 + (oG > ALPHA_MAX ? 1ull << 40 : 0));
     if (pass) pass->push_back(Passing{k + 1, id, alpha, G, T, a, dx, dy, oG > ALPHA_MAX});
-    *last = k + 1;
     T = Tn;
   }
   *margin = mg;
@@ -344,8 +346,8 @@ static double walk_pixel(double px, double py, const uint32_t* ids, uint32_t n, 
 }
 
 // O10 forward: image = sum M_i c_i alpha_i T_i (Eq. 3) + T_{N+1} bg (Eq. 9-10).
-// image [3][H][W], final_T [H][W], n_contrib [H][W] (1-based position of the last blended entry,
-// masked or not), margin [H][W], hash [H][W], counts[2] = {pair evaluations, blends}.
+// image [3][H][W], final_T [H][W], n_contrib [H][W] (number of list entries consumed before the stop,
+// reading 5), margin [H][W], hash [H][W], counts[2] = {pair evaluations, blends}.
 int orc_render_fwd(const Cam* cam, const uint32_t* sorted_ids, const uint32_t* tile_ranges, const double* means2d,
                    const double* conic_opacity, const double* rgb, const float* masks, double* image, double* final_T,
                    uint32_t* n_contrib, double* margin, uint64_t* hash, uint64_t* counts) {

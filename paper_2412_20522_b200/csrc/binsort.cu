@@ -30,10 +30,16 @@
 namespace {
 
 // ---------------------------------------------------------------- S1: radix sort of the N depth keys
-constexpr int RS_THREADS = 512;
-constexpr int RS_ITEMS = 16;
+#ifndef RS_THREADS_
+#define RS_THREADS_ 512
+#endif
+#ifndef RS_ITEMS_
+#define RS_ITEMS_ 8
+#endif
+constexpr int RS_THREADS = RS_THREADS_;
+constexpr int RS_ITEMS = RS_ITEMS_;
 constexpr int RS_WARPS = RS_THREADS / 32;
-constexpr int RS_TILE = RS_THREADS * RS_ITEMS;  // 8192 elements per block
+constexpr int RS_TILE = RS_THREADS * RS_ITEMS;  // 4096 elements per block: 41 KB of shared memory, 5 blocks per SM
 constexpr int RS_BINS = 256;
 
 constexpr int XP_CHUNK = 512;   // items per warp in the expansion sweeps
@@ -63,61 +69,123 @@ struct SortCtl {            // lives in the workspace; zeroed at the start of ev
   uint32_t class_cursor[TO_CLASSES];  // tiles of the class already placed
 };
 
-// One stable radix pass on 8 bits at `shift`.  kCount: write the per-block digit histogram to
-// table[digit][block].  Otherwise: table holds the exclusive scan (digit-major) and the block
-// scatters its elements, keeping their order within a digit.
-template <bool kCount>
-__global__ void __launch_bounds__(RS_THREADS) radix_pass_kernel(
+// One stable radix pass on 8 bits at `shift` is two kernels around a table scan.
+// Count: table[digit][block] = number of the block's keys with that digit (shared-memory histogram).
+__global__ void __launch_bounds__(RS_THREADS) radix_count_kernel(const uint32_t* __restrict__ keys_in, uint32_t n, int shift,
+                                                                 uint32_t* __restrict__ table, int nblocks) {
+  __shared__ uint32_t hist[RS_BINS];
+  for (int tile = blockIdx.x; tile < nblocks; tile += gridDim.x) {  // nblocks = logical tiles of RS_TILE keys
+    if (threadIdx.x < RS_BINS) hist[threadIdx.x] = 0;
+    __syncthreads();
+    const uint32_t base = tile * (uint32_t)RS_TILE;
+#pragma unroll
+    for (int it = 0; it < RS_ITEMS; it++) {
+      const uint32_t idx = base + it * RS_THREADS + threadIdx.x;
+      if (idx < n) atomicAdd(&hist[(keys_in[idx] >> shift) & 255u], 1u);
+    }
+    __syncthreads();
+    if (threadIdx.x < RS_BINS) table[(size_t)threadIdx.x * nblocks + tile] = hist[threadIdx.x];
+  }
+}
+
+// Scatter: table holds the exclusive scan (digit-major).  The block ranks its keys (per-warp match_any
+// counters, warps in order), moves keys and values into digit order in shared memory, and writes them
+// out from there, so that consecutive threads write consecutive addresses of a digit's run: scattered
+// 4-byte stores cost one L2 transaction each and were the bottleneck of this pass.
+struct RadixSmem {
+  uint32_t cnt[RS_WARPS][RS_BINS];  // per-warp digit counts -> exclusive prefix over warps
+  uint32_t lbase[RS_BINS];          // first local position of a digit
+  uint32_t gdelta[RS_BINS];         // global position of a digit's first key minus its local position
+  uint32_t keys[RS_TILE];
+  uint32_t vals[RS_TILE];
+};
+
+__global__ void __launch_bounds__(RS_THREADS) radix_scatter_kernel(
     const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in, uint32_t* __restrict__ keys_out,
-    uint32_t* __restrict__ vals_out, uint32_t n, int shift, uint32_t* __restrict__ table, int nblocks) {
-  __shared__ uint32_t cnt[RS_WARPS][RS_BINS];
-  __shared__ uint32_t gbase[RS_BINS];
+    uint32_t* __restrict__ vals_out, uint32_t n, int shift, const uint32_t* __restrict__ table, int nblocks) {
+  extern __shared__ __align__(16) unsigned char rs_smem_raw[];
+  RadixSmem& sm = *reinterpret_cast<RadixSmem*>(rs_smem_raw);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  for (int i = threadIdx.x; i < RS_WARPS * RS_BINS; i += RS_THREADS) (&cnt[0][0])[i] = 0;
-  __syncthreads();
-  const uint32_t base = blockIdx.x * (uint32_t)RS_TILE + warp * (32 * RS_ITEMS);
-  uint32_t key[RS_ITEMS], rank[RS_ITEMS];
+  for (int tile = blockIdx.x; tile < nblocks; tile += gridDim.x) {  // nblocks = logical tiles of RS_TILE keys
+    for (int i = threadIdx.x; i < RS_WARPS * RS_BINS; i += RS_THREADS) (&sm.cnt[0][0])[i] = 0;
+    __syncthreads();
+    const uint32_t base = tile * (uint32_t)RS_TILE + warp * (32 * RS_ITEMS);
+    uint32_t key[RS_ITEMS], val[RS_ITEMS], rank[RS_ITEMS];
 #pragma unroll
-  for (int it = 0; it < RS_ITEMS; it++) {
-    const uint32_t idx = base + it * 32 + lane;
-    key[it] = idx < n ? keys_in[idx] : 0u;
-  }
-#pragma unroll
-  for (int it = 0; it < RS_ITEMS; it++) {
-    const uint32_t idx = base + it * 32 + lane;
-    const bool valid = idx < n;
-    const uint32_t d = valid ? ((key[it] >> shift) & 255u) : 256u;  // invalid lanes match only each other
-    const uint32_t peers = __match_any_sync(0xffffffffu, d);
-    uint32_t before = 0;
-    if (valid) before = cnt[warp][d];
-    __syncwarp();
-    if (valid && lane == __ffs(peers) - 1) cnt[warp][d] = before + __popc(peers);
-    __syncwarp();
-    rank[it] = before + __popc(peers & ((1u << lane) - 1u));
-  }
-  __syncthreads();
-  if (threadIdx.x < RS_BINS) {
-    uint32_t s = 0;
-#pragma unroll
-    for (int w = 0; w < RS_WARPS; w++) {
-      const uint32_t c = cnt[w][threadIdx.x];
-      cnt[w][threadIdx.x] = s;
-      s += c;
+    for (int it = 0; it < RS_ITEMS; it++) {
+      const uint32_t idx = base + it * 32 + lane;
+      key[it] = idx < n ? keys_in[idx] : 0u;
+      val[it] = (vals_in && idx < n) ? vals_in[idx] : idx;  // first pass: the value is the index itself
     }
-    if (kCount) table[(size_t)threadIdx.x * nblocks + blockIdx.x] = s;
-    else gbase[threadIdx.x] = table[(size_t)threadIdx.x * nblocks + blockIdx.x];
-  }
-  if (kCount) return;
-  __syncthreads();
 #pragma unroll
-  for (int it = 0; it < RS_ITEMS; it++) {
-    const uint32_t idx = base + it * 32 + lane;
-    if (idx < n) {
-      const uint32_t d = (key[it] >> shift) & 255u;
-      const uint32_t dst = gbase[d] + cnt[warp][d] + rank[it];
-      keys_out[dst] = key[it];
-      vals_out[dst] = vals_in ? vals_in[idx] : idx;  // first pass: the value is the index itself
+    for (int it = 0; it < RS_ITEMS; it++) {
+      const uint32_t idx = base + it * 32 + lane;
+      const bool valid = idx < n;
+      const uint32_t d = valid ? ((key[it] >> shift) & 255u) : 256u;  // invalid lanes match only each other
+      const uint32_t peers = __match_any_sync(0xffffffffu, d);
+      uint32_t before = 0;
+      if (valid) before = sm.cnt[warp][d];
+      __syncwarp();
+      if (valid && lane == __ffs(peers) - 1) sm.cnt[warp][d] = before + __popc(peers);
+      __syncwarp();
+      rank[it] = before + __popc(peers & ((1u << lane) - 1u));
     }
+    __syncthreads();
+    // exclusive prefix over warps per digit, digit totals, then an exclusive scan over the 256 digits
+    uint32_t total = 0;
+    if (threadIdx.x < RS_BINS) {
+#pragma unroll
+      for (int w = 0; w < RS_WARPS; w++) {
+        const uint32_t c = sm.cnt[w][threadIdx.x];
+        sm.cnt[w][threadIdx.x] = total;
+        total += c;
+      }
+    }
+    {
+      // threads 0..255 = warps 0..7 hold the totals; warp-level inclusive scan + warp sums via lbase as scratch
+      uint32_t inc = total;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+      }
+      if (threadIdx.x < RS_BINS && lane == 31) sm.gdelta[warp] = inc;  // scratch: sums of warps 0..7
+      __syncthreads();
+      if (threadIdx.x < RS_BINS) {
+        uint32_t woff = 0;
+#pragma unroll
+        for (int w = 0; w < RS_BINS / 32; w++)
+          if (w < warp) woff += sm.gdelta[w];
+        sm.lbase[threadIdx.x] = woff + inc - total;
+      }
+      __syncthreads();
+      if (threadIdx.x < RS_BINS) sm.gdelta[threadIdx.x] = table[(size_t)threadIdx.x * nblocks + tile] - sm.lbase[threadIdx.x];
+    }
+    __syncthreads();
+    // into digit order in shared memory
+#pragma unroll
+    for (int it = 0; it < RS_ITEMS; it++) {
+      const uint32_t idx = base + it * 32 + lane;
+      if (idx < n) {
+        const uint32_t d = (key[it] >> shift) & 255u;
+        const uint32_t lpos = sm.lbase[d] + sm.cnt[warp][d] + rank[it];
+        sm.keys[lpos] = key[it];
+        sm.vals[lpos] = val[it];
+      }
+    }
+    __syncthreads();
+    const uint32_t nblk = min((uint32_t)RS_TILE, n - tile * (uint32_t)RS_TILE);
+#pragma unroll
+    for (int it = 0; it < RS_ITEMS; it++) {
+      const uint32_t j = it * RS_THREADS + threadIdx.x;
+      if (j < nblk) {
+        const uint32_t k = sm.keys[j];
+        const uint32_t dst = sm.gdelta[(k >> shift) & 255u] + j;
+        keys_out[dst] = k;
+        vals_out[dst] = sm.vals[j];
+      }
+    }
+    __syncthreads();  // shared memory is reused by the next tile
   }
 }
 
@@ -598,15 +666,29 @@ extern "C" int mg_bin_sort(const mg_camera* cam, int64_t N, const float* depths,
   }
 
   // S1: depth order of the N Gaussians (culled ones last), R, nvis, overflow flag
+  // radix passes run as persistent grids (one wave of resident blocks looping over the logical tiles)
+  static int rs_grid_count = 0, rs_grid_scatter = 0;
+  if (rs_grid_scatter == 0) {
+    MG_CHECK_CUDA(cudaFuncSetAttribute(radix_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(RadixSmem)));
+    int dev = 0, sms = 0, occ_c = 0, occ_s = 0;
+    MG_CHECK_CUDA(cudaGetDevice(&dev));
+    MG_CHECK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    MG_CHECK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_c, radix_count_kernel, RS_THREADS, 0));
+    MG_CHECK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_s, radix_scatter_kernel, RS_THREADS, sizeof(RadixSmem)));
+    rs_grid_count = sms * (occ_c > 0 ? occ_c : 1);
+    rs_grid_scatter = sms * (occ_s > 0 ? occ_s : 1);
+  }
+  const int grid_c = L.nblk_sort < rs_grid_count ? L.nblk_sort : rs_grid_count;
+  const int grid_s = L.nblk_sort < rs_grid_scatter ? L.nblk_sort : rs_grid_scatter;
   depth_keys_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(N, depths, tiles_touched, keysA, ctl);
   ctl_finalize_kernel<<<1, 1, 0, st>>>(ctl, (unsigned long long)R_capacity);
   MG_CHECK_LAUNCH();
   {
     uint32_t *ki = keysA, *vi = nullptr, *ko = keysB, *vo = valsB;
     for (int pass = 0; pass < 4; pass++) {
-      radix_pass_kernel<true><<<L.nblk_sort, RS_THREADS, 0, st>>>(ki, vi, ko, vo, (uint32_t)N, 8 * pass, table_n, L.nblk_sort);
+      radix_count_kernel<<<grid_c, RS_THREADS, 0, st>>>(ki, (uint32_t)N, 8 * pass, table_n, L.nblk_sort);
       if (int rc = scan_table(table_n, (uint32_t)(RS_BINS * L.nblk_sort), nullptr, (uint32_t)(RS_BINS * L.nblk_sort), sums, st)) return rc;
-      radix_pass_kernel<false><<<L.nblk_sort, RS_THREADS, 0, st>>>(ki, vi, ko, vo, (uint32_t)N, 8 * pass, table_n, L.nblk_sort);
+      radix_scatter_kernel<<<grid_s, RS_THREADS, sizeof(RadixSmem), st>>>(ki, vi, ko, vo, (uint32_t)N, 8 * pass, table_n, L.nblk_sort);
       MG_CHECK_LAUNCH();
       ki = (pass & 1) ? keysA : keysB;
       vi = (pass & 1) ? valsA : valsB;

@@ -8,8 +8,9 @@
 //    mask per entry (lanes = entries), a ballot, then the surviving entries in list order;
 //  * per surviving entry only the reachable, still-live sub-blocks are evaluated; the alpha filter is two
 //    compares on the exponent, the exponential is taken only for pairs that pass;
-//  * an entry with M = 0 changes neither C nor T: for it only the last-contributor index is
-//    updated -- a warp-uniform branch, since M belongs to the entry;
+//  * an entry with M = 0 changes neither C nor T and cannot stop a pixel, and n_contrib counts
+//    the entries consumed before the stop (include/mg.h, reading 5), so masked entries are dropped when the
+//    batch is staged: the forward pass costs nothing for them;
 //  * a warp leaves when all its pixels have stopped.
 #include "render_common.cuh"
 
@@ -47,7 +48,7 @@ __global__ void __launch_bounds__(RN_THREADS, RN_FWD_MINB) render_fwd_kernel(
   uint32_t live = 0;  // bit k set = pixel k still running.  Pixels outside the image never run.
 #pragma unroll
   for (int k = 0; k < 4; k++) {
-    T[k] = 1.f; Cr[k] = Cg[k] = Cb[k] = 0.f; last[k] = 0u;
+    T[k] = 1.f; Cr[k] = Cg[k] = Cb[k] = 0.f; last[k] = (uint32_t)n;  // entries consumed unless a stop says less
     if (px[k & 1] < W && py[k >> 1] < H) live |= 1u << k;
   }
   uint32_t live_sb = 0;  // warp-uniform: bit k set = sub-block k has a running pixel
@@ -67,7 +68,8 @@ __global__ void __launch_bounds__(RN_THREADS, RN_FWD_MINB) render_fwd_kernel(
       uint32_t m4 = 0;
       if (base + lane < n) {
         RnRecord rec = rn_make_record(rn_stage_read(stage, lane));
-        m4 = rn_subblock_mask(rec.a, rec.b, X0, Y0) & live_sb;
+        // an entry with M = 0 changes neither C nor T and cannot stop a pixel: dropped here
+        if (rec.b.z != 0.f) m4 = rn_subblock_mask(rec.a, rec.b, X0, Y0) & live_sb;
         rec.c.w = __uint_as_float(m4);
         buf[lane] = rec;
       }
@@ -85,16 +87,7 @@ __global__ void __launch_bounds__(RN_THREADS, RN_FWD_MINB) render_fwd_kernel(
         const float lo = rb.y, m = rb.z;
         const uint32_t pos = (uint32_t)(base + jj + 1);
         const RnPartial p = rn_partial(ra, rb, fx, fy);
-        if (m == 0.f) {
-          // masked entry: a = 0, so C and T are unchanged and the pixel cannot stop here
-#pragma unroll
-          for (int k = 0; k < 4; k++) {
-            if ((sb >> k) & 1u) {
-              const float e = rn_eval(p, ra.w, k);
-              if (rn_filter(e, lo) && ((live >> k) & 1u)) last[k] = pos;
-            }
-          }
-        } else {
+        {
 #pragma unroll
           for (int k = 0; k < 4; k++) {
             if ((sb >> k) & 1u) {
@@ -106,14 +99,14 @@ __global__ void __launch_bounds__(RN_THREADS, RN_FWD_MINB) render_fwd_kernel(
                   const float a = m * alpha;
                   const float Tn = T[k] * (1.f - a);
                   if (Tn < MG_T_MIN) {
-                    live &= ~(1u << k);  // stop: this entry is neither blended nor counted
+                    live &= ~(1u << k);  // stop: this entry is not blended; pos - 1 entries were consumed
+                    last[k] = pos - 1;
                   } else {
                     const float w = a * T[k];
                     Cr[k] = fmaf(w, rc.x, Cr[k]);
                     Cg[k] = fmaf(w, rc.y, Cg[k]);
                     Cb[k] = fmaf(w, rc.z, Cb[k]);
                     T[k] = Tn;
-                    last[k] = pos;
                   }
                 }
               }

@@ -57,8 +57,7 @@ def np_pixel(px, py, ids, m2, co, rgb, m, bg, masked=True):
     w = (a * Ti)[:n]
     col = (w[:, None] * rgb[ids[:n]]).sum(0)
     Tfin = Tn[n - 1] if n > 0 else 1.0
-    okn = np.nonzero(ok[:n])[0]
-    last = okn[-1] + 1 if len(okn) else 0
+    last = n  # entries consumed: those in front of the stopping entry, or the whole list (reading 5)
     return col + Tfin * np.array(bg, float), Tfin, last, alpha[:n], Ti[:n], ok[:n]
 
 
