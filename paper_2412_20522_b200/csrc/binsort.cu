@@ -17,11 +17,13 @@
 //
 // S2 and S3 are the same primitive, a STABLE INTERVAL EXPANSION: items in sequence order, each with
 // an interval of bins, are appended to every bin of their interval, order preserved.  A warp takes
-// a chunk of 512 consecutive items, 32 at a time: lane k turns its interval into a row of a 32 x
-// 32-bin bit matrix, a 5-stage shuffle butterfly transposes it, and lane c then holds the set of
-// items that cover bin c, in item order.  Counting is a popc; emitting walks the set bits.  Per
-// chunk and bin the counts go to a table, an exclusive scan of the table (bin-major, chunk-minor)
-// gives every (bin, chunk) its write position, and a second sweep emits.
+// a chunk of 512 consecutive items, 32 at a time.  Counting: a difference array per chunk in shared
+// memory (two atomics per item), scanned over the bins at the end.  Per chunk and bin the counts go
+// to a table, an exclusive scan of the table (bin-major, chunk-minor) gives every (bin, chunk) its
+// write position, and a second sweep emits: lane k turns its interval into a row of a 32 x 32-bin bit
+// matrix, a 5-stage shuffle butterfly transposes it, and lane c then holds the set of items that cover
+// bin c, in item order, and walks the set bits.  (A lanes-as-keys variant -- binary search over the
+// scanned widths, then ranking by match -- was measured 1.5x slower: longer dependent chains.)
 //
 // Bytes moved per duplicated key: ~4 B written + ~16 B of records and tables (mostly L2 hits),
 // against ~150 B for six 64-bit key-value radix passes over R keys.
@@ -58,6 +60,19 @@ __device__ __forceinline__ uint32_t length_class(uint32_t n) {
   return 1u + 8u * (uint32_t)msb + frac;
 }
 
+// Lanes with the same `nbits`-bit value among the lanes of `vmask` (the caller's own lane included), built
+// from one ballot per bit.  On sm_100a this is several times faster than match.any, whose cost made it the
+// bottleneck of every ranking loop here.
+__device__ __forceinline__ uint32_t peers_by_ballot(uint32_t v, int nbits, uint32_t vmask) {
+  uint32_t peers = vmask;
+  for (int b = 0; b < nbits; b++) {
+    const bool bit = (v >> b) & 1u;
+    const uint32_t set = __ballot_sync(0xffffffffu, bit);
+    peers &= bit ? set : ~set;
+  }
+  return peers;
+}
+
 struct SortCtl {            // lives in the workspace; zeroed at the start of every call
   unsigned long long R;     // true number of duplicated keys = sum of tiles_touched
   uint32_t nvis;            // Gaussians with tiles_touched > 0
@@ -88,7 +103,7 @@ __global__ void __launch_bounds__(RS_THREADS) radix_count_kernel(const uint32_t*
   }
 }
 
-// Scatter: table holds the exclusive scan (digit-major).  The block ranks its keys (per-warp match_any
+// Scatter: table holds the exclusive scan (digit-major).  The block ranks its keys (per-warp digit
 // counters, warps in order), moves keys and values into digit order in shared memory, and writes them
 // out from there, so that consecutive threads write consecutive addresses of a digit's run: scattered
 // 4-byte stores cost one L2 transaction each and were the bottleneck of this pass.
@@ -121,8 +136,8 @@ __global__ void __launch_bounds__(RS_THREADS) radix_scatter_kernel(
     for (int it = 0; it < RS_ITEMS; it++) {
       const uint32_t idx = base + it * 32 + lane;
       const bool valid = idx < n;
-      const uint32_t d = valid ? ((key[it] >> shift) & 255u) : 256u;  // invalid lanes match only each other
-      const uint32_t peers = __match_any_sync(0xffffffffu, d);
+      const uint32_t d = (key[it] >> shift) & 255u;
+      const uint32_t peers = peers_by_ballot(d, 8, __ballot_sync(0xffffffffu, valid));
       uint32_t before = 0;
       if (valid) before = sm.cnt[warp][d];
       __syncwarp();
@@ -311,6 +326,32 @@ __global__ void __launch_bounds__(SCAN_THREADS) scan_apply_kernel(uint32_t* __re
 }
 
 // ---------------------------------------------------------------- stable interval expansion
+// Counting sweep, per warp and group of 32 items: a difference array in shared memory (+1 at lo, -1 at hi,
+// two atomics per ITEM, not per key); xp_counts_to_table turns it into per-bin counts at the end of the chunk.
+__device__ __forceinline__ void xp_count_group(int lo, int hi, uint32_t* cnt) {
+  if (hi > lo) {
+    atomicAdd(&cnt[lo], 1u);
+    atomicSub(&cnt[hi], 1u);  // cnt has bins + 1 entries
+  }
+}
+
+// Inclusive scan of the difference array over the bins -> counts; written to table[b * stride] (b < bins).
+__device__ __forceinline__ void xp_counts_to_table(const uint32_t* cnt, int bins, int lane, uint32_t* table, size_t stride) {
+  uint32_t carry = 0;
+  for (int b0 = 0; b0 < bins; b0 += 32) {
+    const int b = b0 + lane;
+    uint32_t v = b < bins ? cnt[b] : 0u;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t t = __shfl_up_sync(0xffffffffu, v, o);
+      if (lane >= o) v += t;
+    }
+    v += carry;
+    if (b < bins) table[(size_t)b * stride] = v;
+    carry = __shfl_sync(0xffffffffu, v, 31);
+  }
+}
+
 // Bits [lo, hi) of the 32-bin word w.
 __device__ __forceinline__ uint32_t interval_bits(int lo, int hi, int w) {
   const int l = max(lo - 32 * w, 0), h = min(hi - 32 * w, 32);
@@ -339,6 +380,35 @@ __device__ __forceinline__ void word_range(int lo, int hi, int* wlo, int* whi) {
   *whi = (int)__reduce_max_sync(0xffffffffu, any ? (hi - 1) >> 5 : -1);
 }
 
+// Emitting sweep, per warp and group of 32 items (lane k holds item k: interval [lo, hi), payload p0 and, if
+// kWords == 2, p1): lane k turns its interval into a row of a 32 x 32-bin bit matrix per 32-bin word, a
+// 5-stage shuffle butterfly transposes it, and lane c then holds the set of items that cover bin c, in
+// item order; it walks the set bits and appends the payloads at the bin's write cursor cnt[bin].
+template <int kWords>
+__device__ __forceinline__ void xp_emit_group(int lo, int hi, uint32_t p0, uint32_t p1, uint32_t* cnt, int lane,
+                                              uint32_t* __restrict__ out) {
+  int wlo, whi;
+  word_range(lo, hi, &wlo, &whi);
+  for (int w = wlo; w <= whi; w++) {
+    uint32_t col = transpose32(interval_bits(lo, hi, w), lane);
+    const int bin = 32 * w + lane;
+    const bool mine = col != 0;  // implies bin < bins
+    uint32_t p = mine ? cnt[bin] : 0u;
+    while (__any_sync(0xffffffffu, col != 0)) {
+      const int src = col ? __ffs(col) - 1 : 0;
+      const uint32_t v0 = __shfl_sync(0xffffffffu, p0, src);
+      uint32_t v1 = 0;
+      if (kWords == 2) v1 = __shfl_sync(0xffffffffu, p1, src);
+      if (col) {
+        if (kWords == 2) reinterpret_cast<uint2*>(out)[p++] = make_uint2(v0, v1);
+        else out[p++] = v0;
+        col &= col - 1;
+      }
+    }
+    if (mine) cnt[bin] = p;
+  }
+}
+
 // S2: row expansion.  Item k of the depth order (k < nvis) covers rows [y0, y1).
 // kCount: table_r[row * n_chunks + chunk] = number of records of this chunk in that row; also stores the
 // packed rectangle in depth order for the second sweep.  Otherwise table_r is scanned and the records
@@ -353,10 +423,10 @@ __global__ void __launch_bounds__(32 * XP_MAX_WARPS) row_expand_kernel(
   const uint32_t chunk = blockIdx.x * (uint32_t)warps_per_block + warp;
   if (chunk >= n_chunks) return;
   if (!kCount && ctl->overflow) return;
-  uint32_t* cnt = xp_smem + (size_t)warp * gh;
+  uint32_t* cnt = xp_smem + (size_t)warp * (gh + 1);
   const uint32_t nvis = ctl->nvis;
   const uint32_t k0 = chunk * (uint32_t)XP_CHUNK;
-  for (int b = lane; b < gh; b += 32) cnt[b] = kCount ? 0u : table_r[(size_t)b * n_chunks + chunk];
+  for (int b = lane; b <= gh; b += 32) cnt[b] = (kCount || b == gh) ? 0u : table_r[(size_t)b * n_chunks + chunk];
   __syncwarp();
   if (k0 < nvis) {
     const uint32_t k1 = min(k0 + (uint32_t)XP_CHUNK, nvis);
@@ -365,45 +435,26 @@ __global__ void __launch_bounds__(32 * XP_MAX_WARPS) row_expand_kernel(
       uint32_t id = 0, xx = 0;
       int lo = 0, hi = 0;
       if (k < k1) {
-        id = order[k];
         if (kCount) {
+          id = order[k];
           const int4 r = rects[id];
           xx = (uint32_t)r.x | ((uint32_t)r.z << 16);
           lo = r.y; hi = r.w;
           prect[k] = make_uint2(xx, (uint32_t)r.y | ((uint32_t)r.w << 16));
         } else {
+          id = order[k];
           const uint2 p = prect[k];
           xx = p.x;
           lo = (int)(p.y & 0xffffu); hi = (int)(p.y >> 16);
         }
       }
-      int wlo, whi;
-      word_range(lo, hi, &wlo, &whi);
-      for (int w = wlo; w <= whi; w++) {
-        uint32_t col = transpose32(interval_bits(lo, hi, w), lane);
-        const int bin = 32 * w + lane;
-        if (kCount) {
-          if (col) cnt[bin] += __popc(col);  // col != 0 implies bin < gh
-        } else {
-          uint32_t p = col ? cnt[bin] : 0u;
-          const bool mine = col != 0;
-          while (__any_sync(0xffffffffu, col != 0)) {
-            const int src = col ? __ffs(col) - 1 : 0;
-            const uint32_t vid = __shfl_sync(0xffffffffu, id, src);
-            const uint32_t vxx = __shfl_sync(0xffffffffu, xx, src);
-            if (col) {
-              row_rec[p++] = make_uint2(vid, vxx);
-              col &= col - 1;
-            }
-          }
-          if (mine) cnt[bin] = p;
-        }
-      }
+      if (kCount) xp_count_group(lo, hi, cnt);
+      else xp_emit_group<2>(lo, hi, id, xx, cnt, lane, reinterpret_cast<uint32_t*>(row_rec));
     }
   }
   if (kCount) {
     __syncwarp();
-    for (int b = lane; b < gh; b += 32) table_r[(size_t)b * n_chunks + chunk] = cnt[b];
+    xp_counts_to_table(cnt, gh, lane, table_r + chunk, n_chunks);
   }
 }
 
@@ -456,7 +507,7 @@ __global__ void __launch_bounds__(32 * XP_MAX_WARPS) col_expand_kernel(
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t g = blockIdx.x * (uint32_t)warps_per_block + warp;
   if (g >= ctl->n_chunks_c) return;
-  uint32_t* cnt = xp_smem + (size_t)warp * gw;
+  uint32_t* cnt = xp_smem + (size_t)warp * (gw + 1);
   // row of this chunk: the last r with chunk_base[r] <= g
   int lo_r = 0, hi_r = gh;  // invariant: chunk_base[lo_r] <= g < chunk_base[hi_r]
   while (hi_r - lo_r > 1) {
@@ -468,7 +519,7 @@ __global__ void __launch_bounds__(32 * XP_MAX_WARPS) col_expand_kernel(
   const uint32_t j0 = row_start[r] + c * (uint32_t)XP_CHUNK;
   const uint32_t j1 = min(j0 + (uint32_t)XP_CHUNK, row_start[r + 1]);
   uint32_t* tab = table_c + (size_t)gw * cb + c;
-  for (int b = lane; b < gw; b += 32) cnt[b] = kCount ? 0u : tab[(size_t)b * nch];
+  for (int b = lane; b <= gw; b += 32) cnt[b] = (kCount || b == gw) ? 0u : tab[(size_t)b * nch];
   __syncwarp();
   for (uint32_t jb = j0; jb < j1; jb += 32) {
     const uint32_t j = jb + lane;
@@ -479,31 +530,12 @@ __global__ void __launch_bounds__(32 * XP_MAX_WARPS) col_expand_kernel(
       id = rec.x;
       lo = (int)(rec.y & 0xffffu); hi = (int)(rec.y >> 16);
     }
-    int wlo, whi;
-    word_range(lo, hi, &wlo, &whi);
-    for (int w = wlo; w <= whi; w++) {
-      uint32_t col = transpose32(interval_bits(lo, hi, w), lane);
-      const int bin = 32 * w + lane;
-      if (kCount) {
-        if (col) cnt[bin] += __popc(col);
-      } else {
-        uint32_t p = col ? cnt[bin] : 0u;
-        const bool mine = col != 0;
-        while (__any_sync(0xffffffffu, col != 0)) {
-          const int src = col ? __ffs(col) - 1 : 0;
-          const uint32_t vid = __shfl_sync(0xffffffffu, id, src);
-          if (col) {
-            sorted_ids[p++] = vid;
-            col &= col - 1;
-          }
-        }
-        if (mine) cnt[bin] = p;
-      }
-    }
+    if (kCount) xp_count_group(lo, hi, cnt);
+    else xp_emit_group<1>(lo, hi, id, 0u, cnt, lane, sorted_ids);
   }
   if (kCount) {
     __syncwarp();
-    for (int b = lane; b < gw; b += 32) tab[(size_t)b * nch] = cnt[b];
+    xp_counts_to_table(cnt, gw, lane, tab, nch);
   }
 }
 
@@ -700,8 +732,8 @@ extern "C" int mg_bin_sort(const mg_camera* cam, int64_t N, const float* depths,
 
   // S2: row expansion
   {
-    const int wpb = xp_warps(gh);
-    const size_t smem = (size_t)wpb * gh * 4;
+    const int wpb = xp_warps(gh + 1);
+    const size_t smem = (size_t)wpb * (gh + 1) * 4;
     if (int rc = xp_prepare(row_expand_kernel<true>, smem)) return rc;
     if (int rc = xp_prepare(row_expand_kernel<false>, smem)) return rc;
     const unsigned grid = (L.n_chunks_r + wpb - 1) / wpb;
@@ -714,8 +746,8 @@ extern "C" int mg_bin_sort(const mg_camera* cam, int64_t N, const float* depths,
   }
   // S3: column expansion and tile ranges
   {
-    const int wpb = xp_warps(gw);
-    const size_t smem = (size_t)wpb * gw * 4;
+    const int wpb = xp_warps(gw + 1);
+    const size_t smem = (size_t)wpb * (gw + 1) * 4;
     if (int rc = xp_prepare(col_expand_kernel<true>, smem)) return rc;
     if (int rc = xp_prepare(col_expand_kernel<false>, smem)) return rc;
     const unsigned grid = (L.max_chunks_c + wpb - 1) / wpb;
