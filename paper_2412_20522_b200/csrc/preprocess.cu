@@ -1,6 +1,7 @@
 // preprocess.cu -- mg_preprocess: activate + EWA-project + SH colour + 3-sigma tile bounds.
-// Steps a1-a3 of the hot path (PAPER.md:64-66 sec. 3.1, :74; O1-O8).  HBM-bound:
-// one thread per Gaussian, independent 128-bit loads of the SH row issued up front.
+// Steps a1-a3 of the hot path (PAPER.md:64-66 sec. 3.1, :74; O1-O8).  HBM-bound: one thread per
+// Gaussian.  Geometry first (44 B); then the 192-byte SH rows of the VISIBLE Gaussians only, read with
+// coalesced 128-bit loads through shared memory (a culled Gaussian never touches its row).
 #include "mg_common.cuh"
 
 namespace {
@@ -34,47 +35,54 @@ __device__ __forceinline__ void sh_basis(float x, float y, float z, float* Y) {
   }
 }
 
+// Floats per SH row, and the row stride in shared memory (128-bit accesses of 8 consecutive lanes cover all
+// banks when stride / 4 is odd; scalar accesses when the stride is odd).
 template <int D>
-__global__ void __launch_bounds__(256) preprocess_kernel(
+struct ShRowLayout {
+  static constexpr int K = (D + 1) * (D + 1);
+  static constexpr int RK = 3 * K;
+  static constexpr bool VEC = (RK % 4) == 0;  // D = 1, 3
+  static constexpr int STRIDE = VEC ? (((RK / 4) % 2) ? RK : RK + 4) : ((RK % 2) ? RK : RK + 1);
+};
+
+constexpr int PP_THREADS = 128;
+
+template <int D>
+__global__ void __launch_bounds__(PP_THREADS) preprocess_kernel(
     mg_camera cam, int64_t N, const float* __restrict__ means, const float* __restrict__ log_scales,
     const float* __restrict__ quats, const float* __restrict__ opacity_logits, const float* __restrict__ sh,
     float2* __restrict__ means2d, float* __restrict__ depths, float4* __restrict__ conic_opacity,
     float* __restrict__ rgb, int32_t* __restrict__ radii, int4* __restrict__ rects,
     uint32_t* __restrict__ tiles_touched, uint8_t* __restrict__ clamped) {
-  constexpr int K = (D + 1) * (D + 1);
+  typedef ShRowLayout<D> L;
+  constexpr int K = L::K, RK = L::RK, STRIDE = L::STRIDE;
+  __shared__ __align__(16) float rows_all[PP_THREADS / 32][32 * STRIDE];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  float* wrow = rows_all[warp];
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t g0 = i - lane;  // first Gaussian of this warp
+  const int nrows = (int)max((int64_t)0, min((int64_t)32, N - g0));
   uint32_t touched = 0;
+  // results of the geometry phase, stored after the colour phase
+  float2 m2 = make_float2(0.f, 0.f);
+  float4 co = make_float4(0.f, 0.f, 0.f, 0.f);
+  float col[3] = {0.f, 0.f, 0.f};
+  int radius = 0;
+  int4 rect = make_int4(0, 0, 0, 0);
+  uint32_t clampbits = 0;
+  float tz = 0.f, dirx = 0.f, diry = 0.f, dirz = 0.f;
   if (i < N) {
-    // SH row first: the longest-latency loads go out before the geometry arithmetic
-    float shv[3 * K];
-    const float* shrow = sh + i * (3 * K);
-    if ((3 * K) % 4 == 0) {
-#pragma unroll
-      for (int j = 0; j < 3 * K / 4; j++) {
-        const float4 v = __ldg(reinterpret_cast<const float4*>(shrow) + j);
-        shv[4 * j] = v.x; shv[4 * j + 1] = v.y; shv[4 * j + 2] = v.z; shv[4 * j + 3] = v.w;
-      }
-    } else {
-#pragma unroll
-      for (int j = 0; j < 3 * K; j++) shv[j] = __ldg(shrow + j);
-    }
     const float px = means[3 * i], py = means[3 * i + 1], pz = means[3 * i + 2];
     const float4 q = __ldg(reinterpret_cast<const float4*>(quats) + i);
     const float ls0 = log_scales[3 * i], ls1 = log_scales[3 * i + 1], ls2 = log_scales[3 * i + 2];
     const float logit = opacity_logits[i];
     const float* R = cam.R;
 
-    float2 m2 = make_float2(0.f, 0.f);
-    float4 co = make_float4(0.f, 0.f, 0.f, 0.f);
-    float col[3] = {0.f, 0.f, 0.f};
-    int radius = 0;
-    int4 rect = make_int4(0, 0, 0, 0);
-    uint32_t clampbits = 0;
 
     // O2 camera space
     const float tx = R[0] * px + R[1] * py + R[2] * pz + cam.t[0];
     const float ty = R[3] * px + R[4] * py + R[5] * pz + cam.t[1];
-    const float tz = R[6] * px + R[7] * py + R[8] * pz + cam.t[2];
+    tz = R[6] * px + R[7] * py + R[8] * pz + cam.t[2];
     if (tz > MG_ZNEAR) {
       // O1 activations, O3 Sigma = M M^T with M = Rot diag(s)
       const float s0 = expf(ls0), s1 = expf(ls1), s2 = expf(ls2);
@@ -123,26 +131,63 @@ __global__ void __launch_bounds__(256) preprocess_kernel(
           rect = make_int4(x0, y0, x1, y1);
           m2 = make_float2(mx, my);
           co = make_float4(c * idet, -b * idet, a * idet, 1.f / (1.f + expf(-logit)));
-          // O8 colour along the unit vector camera centre -> Gaussian centre
+          // O8 direction of the unit vector camera centre -> Gaussian centre (colour: second phase)
           const float cpx = -(R[0] * cam.t[0] + R[3] * cam.t[1] + R[6] * cam.t[2]);
           const float cpy = -(R[1] * cam.t[0] + R[4] * cam.t[1] + R[7] * cam.t[2]);
           const float cpz = -(R[2] * cam.t[0] + R[5] * cam.t[1] + R[8] * cam.t[2]);
-          float dx = px - cpx, dy = py - cpy, dz = pz - cpz;
+          const float dx = px - cpx, dy = py - cpy, dz = pz - cpz;
           const float dinv = rsqrtf(dx * dx + dy * dy + dz * dz);
-          dx *= dinv; dy *= dinv; dz *= dinv;
-          float Y[K];
-          sh_basis<D>(dx, dy, dz, Y);
-#pragma unroll
-          for (int k = 0; k < 3; k++) {
-            float v = 0.5f;
-#pragma unroll
-            for (int j = 0; j < K; j++) v = fmaf(Y[j], shv[3 * j + k], v);
-            if (v < 0.f) { v = 0.f; clampbits |= 1u << k; }
-            col[k] = v;
-          }
+          dirx = dx * dinv; diry = dy * dinv; dirz = dz * dinv;
         }
       }
     }
+  }
+  // ---- colour phase: the SH rows of the warp's VISIBLE Gaussians, read by flat position with coalesced
+  // 128-bit loads (a warp's 32 rows are contiguous), staged in shared memory, one row per lane
+  const uint32_t vmask = __ballot_sync(0xffffffffu, touched > 0);
+  if (nrows > 0 && vmask) {
+    if (L::VEC) {
+      const float4* src = reinterpret_cast<const float4*>(sh + g0 * RK);
+#pragma unroll
+      for (int k = 0; k < RK / 4; k++) {
+        const int f = k * 32 + lane, g = f / (RK / 4), c = f % (RK / 4);
+        if (g < nrows && ((vmask >> g) & 1u)) *reinterpret_cast<float4*>(wrow + g * STRIDE + 4 * c) = __ldg(src + f);
+      }
+    } else {
+      const float* src = sh + g0 * RK;
+#pragma unroll
+      for (int k = 0; k < RK; k++) {
+        const int f = k * 32 + lane, g = f / RK, c = f % RK;
+        if (g < nrows && ((vmask >> g) & 1u)) wrow[g * STRIDE + c] = __ldg(src + f);
+      }
+    }
+  }
+  __syncwarp();
+  if (touched > 0) {
+    const float* myrow = wrow + lane * STRIDE;
+    float shv[RK];
+    if (L::VEC) {
+#pragma unroll
+      for (int j = 0; j < RK / 4; j++) {
+        const float4 v = *reinterpret_cast<const float4*>(myrow + 4 * j);
+        shv[4 * j] = v.x; shv[4 * j + 1] = v.y; shv[4 * j + 2] = v.z; shv[4 * j + 3] = v.w;
+      }
+    } else {
+#pragma unroll
+      for (int j = 0; j < RK; j++) shv[j] = myrow[j];
+    }
+    float Y[K];
+    sh_basis<D>(dirx, diry, dirz, Y);
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+      float v = 0.5f;
+#pragma unroll
+      for (int j = 0; j < K; j++) v = fmaf(Y[j], shv[3 * j + k], v);
+      if (v < 0.f) { v = 0.f; clampbits |= 1u << k; }
+      col[k] = v;
+    }
+  }
+  if (i < N) {
     means2d[i] = m2;
     depths[i] = tz;
     conic_opacity[i] = co;
@@ -174,7 +219,7 @@ extern "C" int mg_preprocess(const mg_camera* cam, int64_t N, const float* means
   if (N > 0) {
     MG_REQUIRE(means && log_scales && quats && opacity_logits && sh, "null input array");
     MG_REQUIRE(means2d && depths && conic_opacity && rgb && radii && rects && tiles_touched && clamped, "null output array");
-    const int threads = 256;
+    const int threads = PP_THREADS;
     const unsigned blocks = (unsigned)((N + threads - 1) / threads);
 #define MG_LAUNCH(D)                                                                                              \
   preprocess_kernel<D><<<blocks, threads, 0, st>>>(*cam, N, means, log_scales, quats, opacity_logits, sh,         \
