@@ -31,9 +31,9 @@ if ROOT not in sys.path:
 FLOP_PAIR = 13        # per pair evaluation: 2 sub, 6 quadratic form, mul, min, 2 compares (+1 MUFU not counted)
 FLOP_BLEND_FWD = 11   # per blend, forward
 FLOP_BLEND_BWD = 59   # per blend, backward (49 + 10 adds of the per-entry reduction)
-# kernels of libmg launched per step (memsets and copies not counted): bin_sort = depth keys + ctl + 4 x (count,
-# 2 scan, scatter) + row expansion (count, 2 scan, plan, emit) + column expansion (count, 2 scan, emit, ranges, tile order)
-KERNELS_PER_STEP = {"preprocess": 1, "bin_sort": 2 + 4 * 4 + 5 + 6, "render_fwd": 1, "render_bwd": 1,
+# kernels of libmg launched per step (memsets and copies not counted): bin_sort = depth keys + ctl + 4 single-kernel
+# radix passes + row expansion (count, 2 scan, plan, emit) + column expansion (count, 2 scan, emit, ranges, tile order)
+KERNELS_PER_STEP = {"preprocess": 1, "bin_sort": 2 + 4 + 5 + 6, "render_fwd": 1, "render_bwd": 1,
                     "preprocess_bwd": 2}
 
 

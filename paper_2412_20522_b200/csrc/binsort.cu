@@ -80,33 +80,17 @@ struct SortCtl {            // lives in the workspace; zeroed at the start of ev
   uint32_t n_chunks_c;      // chunks of the column expansion (sum over rows of ceil(records / XP_CHUNK))
   uint32_t n_table_c;       // gw * n_chunks_c
   uint32_t pad[2];
+  uint32_t ticket[4];       // next logical tile of each radix pass (tiles are taken in ticket order)
+  uint32_t spin_fail;       // set if a look-back ever gave up (never in a correct run)
+  uint32_t pad2[3];
+  uint32_t ghist[4][RS_BINS];  // digit histograms of the depth keys, all four passes; then exclusive bases
   uint32_t class_count[TO_CLASSES];   // tiles per list-length class (tile_order)
   uint32_t class_cursor[TO_CLASSES];  // tiles of the class already placed
 };
 
-// One stable radix pass on 8 bits at `shift` is two kernels around a table scan.
-// Count: table[digit][block] = number of the block's keys with that digit (shared-memory histogram).
-__global__ void __launch_bounds__(RS_THREADS) radix_count_kernel(const uint32_t* __restrict__ keys_in, uint32_t n, int shift,
-                                                                 uint32_t* __restrict__ table, int nblocks) {
-  __shared__ uint32_t hist[RS_BINS];
-  for (int tile = blockIdx.x; tile < nblocks; tile += gridDim.x) {  // nblocks = logical tiles of RS_TILE keys
-    if (threadIdx.x < RS_BINS) hist[threadIdx.x] = 0;
-    __syncthreads();
-    const uint32_t base = tile * (uint32_t)RS_TILE;
-#pragma unroll
-    for (int it = 0; it < RS_ITEMS; it++) {
-      const uint32_t idx = base + it * RS_THREADS + threadIdx.x;
-      if (idx < n) atomicAdd(&hist[(keys_in[idx] >> shift) & 255u], 1u);
-    }
-    __syncthreads();
-    if (threadIdx.x < RS_BINS) table[(size_t)threadIdx.x * nblocks + tile] = hist[threadIdx.x];
-  }
-}
-
-// Scatter: table holds the exclusive scan (digit-major).  The block ranks its keys (per-warp digit
-// counters, warps in order), moves keys and values into digit order in shared memory, and writes them
-// out from there, so that consecutive threads write consecutive addresses of a digit's run: scattered
-// 4-byte stores cost one L2 transaction each and were the bottleneck of this pass.
+// Shared memory of a radix pass.  The block ranks its keys (per-warp digit counters, warps in order), moves
+// keys and values into digit order in shared memory, and writes them out from there, so that consecutive
+// threads write consecutive addresses of a digit's run.
 struct RadixSmem {
   uint32_t cnt[RS_WARPS][RS_BINS];  // per-warp digit counts -> exclusive prefix over warps
   uint32_t lbase[RS_BINS];          // first local position of a digit
@@ -115,112 +99,158 @@ struct RadixSmem {
   uint32_t vals[RS_TILE];
 };
 
-__global__ void __launch_bounds__(RS_THREADS) radix_scatter_kernel(
+__device__ __forceinline__ void st_relaxed_u64(unsigned long long* p, unsigned long long v) {
+  asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ unsigned long long ld_relaxed_u64(const unsigned long long* p) {
+  unsigned long long v;
+  asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+  return v;
+}
+
+constexpr unsigned long long LB_AGGREGATE = 1ull << 32;  // status word = flag << 32 | count
+constexpr unsigned long long LB_INCLUSIVE = 2ull << 32;
+constexpr int LB_SPIN_LIMIT = 1 << 26;                   // a look-back that gives up flags ctl->spin_fail
+
+// One radix pass = ONE kernel (single-pass chained scan with decoupled look-back): a block takes the next
+// logical tile by ticket, ranks its 4096 keys, publishes its per-digit counts, and obtains its per-digit
+// offsets by summing the counts its predecessors have published (an "aggregate" if that tile has only
+// counted, an "inclusive" total -- which ends the walk -- once it has finished its own look-back).  Tiles
+// are taken in ticket order, so a block only ever waits for blocks that started before it.  The digit
+// bases of the whole array come from the histograms depth_keys_kernel took.
+__global__ void __launch_bounds__(RS_THREADS) radix_onesweep_kernel(
     const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in, uint32_t* __restrict__ keys_out,
-    uint32_t* __restrict__ vals_out, uint32_t n, int shift, const uint32_t* __restrict__ table, int nblocks) {
+    uint32_t* __restrict__ vals_out, uint32_t n, int pass, SortCtl* __restrict__ ctl,
+    unsigned long long* __restrict__ status) {
   extern __shared__ __align__(16) unsigned char rs_smem_raw[];
   RadixSmem& sm = *reinterpret_cast<RadixSmem*>(rs_smem_raw);
+  __shared__ uint32_t s_tile;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  for (int tile = blockIdx.x; tile < nblocks; tile += gridDim.x) {  // nblocks = logical tiles of RS_TILE keys
-    for (int i = threadIdx.x; i < RS_WARPS * RS_BINS; i += RS_THREADS) (&sm.cnt[0][0])[i] = 0;
-    __syncthreads();
-    const uint32_t base = tile * (uint32_t)RS_TILE + warp * (32 * RS_ITEMS);
-    uint32_t key[RS_ITEMS], val[RS_ITEMS], rank[RS_ITEMS];
+  const int shift = 8 * pass;
+  if (threadIdx.x == 0) s_tile = atomicAdd(&ctl->ticket[pass], 1u);
+  for (int i = threadIdx.x; i < RS_WARPS * RS_BINS; i += RS_THREADS) (&sm.cnt[0][0])[i] = 0;
+  __syncthreads();
+  const uint32_t tile = s_tile;
+  const uint32_t base = tile * (uint32_t)RS_TILE + warp * (32 * RS_ITEMS);
+  uint32_t key[RS_ITEMS], val[RS_ITEMS], rank[RS_ITEMS];
 #pragma unroll
-    for (int it = 0; it < RS_ITEMS; it++) {
-      const uint32_t idx = base + it * 32 + lane;
-      key[it] = idx < n ? keys_in[idx] : 0u;
-      val[it] = (vals_in && idx < n) ? vals_in[idx] : idx;  // first pass: the value is the index itself
-    }
+  for (int it = 0; it < RS_ITEMS; it++) {
+    const uint32_t idx = base + it * 32 + lane;
+    key[it] = idx < n ? keys_in[idx] : 0u;
+    val[it] = (vals_in && idx < n) ? vals_in[idx] : idx;  // first pass: the value is the index itself
+  }
 #pragma unroll
-    for (int it = 0; it < RS_ITEMS; it++) {
-      const uint32_t idx = base + it * 32 + lane;
-      const bool valid = idx < n;
-      const uint32_t d = (key[it] >> shift) & 255u;
-      const uint32_t peers = peers_by_ballot(d, 8, __ballot_sync(0xffffffffu, valid));
-      uint32_t before = 0;
-      if (valid) before = sm.cnt[warp][d];
-      __syncwarp();
-      if (valid && lane == __ffs(peers) - 1) sm.cnt[warp][d] = before + __popc(peers);
-      __syncwarp();
-      rank[it] = before + __popc(peers & ((1u << lane) - 1u));
+  for (int it = 0; it < RS_ITEMS; it++) {
+    const uint32_t idx = base + it * 32 + lane;
+    const bool valid = idx < n;
+    const uint32_t d = (key[it] >> shift) & 255u;
+    const uint32_t peers = peers_by_ballot(d, 8, __ballot_sync(0xffffffffu, valid));
+    uint32_t before = 0;
+    if (valid) before = sm.cnt[warp][d];
+    __syncwarp();
+    if (valid && lane == __ffs(peers) - 1) sm.cnt[warp][d] = before + __popc(peers);
+    __syncwarp();
+    rank[it] = before + __popc(peers & ((1u << lane) - 1u));
+  }
+  __syncthreads();
+  // exclusive prefix over warps per digit; the digit totals are published at once (aggregate)
+  uint32_t total = 0;
+  unsigned long long* my_status = status + (size_t)tile * RS_BINS + threadIdx.x;
+  if (threadIdx.x < RS_BINS) {
+#pragma unroll
+    for (int w = 0; w < RS_WARPS; w++) {
+      const uint32_t c = sm.cnt[w][threadIdx.x];
+      sm.cnt[w][threadIdx.x] = total;
+      total += c;
     }
+    st_relaxed_u64(my_status, LB_AGGREGATE | total);
+  }
+  {
+    // exclusive scan of the totals over the 256 digits -> first local position of a digit
+    uint32_t inc = total;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= o) inc += t;
+    }
+    if (threadIdx.x < RS_BINS && lane == 31) sm.gdelta[warp] = inc;  // scratch: sums of warps 0..7
     __syncthreads();
-    // exclusive prefix over warps per digit, digit totals, then an exclusive scan over the 256 digits
-    uint32_t total = 0;
     if (threadIdx.x < RS_BINS) {
+      uint32_t woff = 0;
 #pragma unroll
-      for (int w = 0; w < RS_WARPS; w++) {
-        const uint32_t c = sm.cnt[w][threadIdx.x];
-        sm.cnt[w][threadIdx.x] = total;
-        total += c;
-      }
-    }
-    {
-      // threads 0..255 = warps 0..7 hold the totals; warp-level inclusive scan + warp sums via lbase as scratch
-      uint32_t inc = total;
-#pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
-        const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
-        if (lane >= o) inc += t;
-      }
-      if (threadIdx.x < RS_BINS && lane == 31) sm.gdelta[warp] = inc;  // scratch: sums of warps 0..7
-      __syncthreads();
-      if (threadIdx.x < RS_BINS) {
-        uint32_t woff = 0;
-#pragma unroll
-        for (int w = 0; w < RS_BINS / 32; w++)
-          if (w < warp) woff += sm.gdelta[w];
-        sm.lbase[threadIdx.x] = woff + inc - total;
-      }
-      __syncthreads();
-      if (threadIdx.x < RS_BINS) sm.gdelta[threadIdx.x] = table[(size_t)threadIdx.x * nblocks + tile] - sm.lbase[threadIdx.x];
+      for (int w = 0; w < RS_BINS / 32; w++)
+        if (w < warp) woff += sm.gdelta[w];
+      sm.lbase[threadIdx.x] = woff + inc - total;
     }
     __syncthreads();
-    // into digit order in shared memory
-#pragma unroll
-    for (int it = 0; it < RS_ITEMS; it++) {
-      const uint32_t idx = base + it * 32 + lane;
-      if (idx < n) {
-        const uint32_t d = (key[it] >> shift) & 255u;
-        const uint32_t lpos = sm.lbase[d] + sm.cnt[warp][d] + rank[it];
-        sm.keys[lpos] = key[it];
-        sm.vals[lpos] = val[it];
-      }
+  }
+  if (threadIdx.x < RS_BINS) {
+    // decoupled look-back over the tiles before this one, one digit per thread
+    uint32_t prefix = 0;
+    for (int t = (int)tile - 1; t >= 0; t--) {
+      const unsigned long long* ps = status + (size_t)t * RS_BINS + threadIdx.x;
+      unsigned long long w = ld_relaxed_u64(ps);
+      int spins = 0;
+      while ((w >> 32) == 0 && ++spins < LB_SPIN_LIMIT) w = ld_relaxed_u64(ps);
+      if ((w >> 32) == 0) { ctl->spin_fail = 1u; break; }
+      prefix += (uint32_t)w;
+      if ((w & LB_INCLUSIVE) != 0) break;
     }
-    __syncthreads();
-    const uint32_t nblk = min((uint32_t)RS_TILE, n - tile * (uint32_t)RS_TILE);
+    st_relaxed_u64(my_status, LB_INCLUSIVE | (unsigned long long)(prefix + total));
+    sm.gdelta[threadIdx.x] = ctl->ghist[pass][threadIdx.x] + prefix - sm.lbase[threadIdx.x];
+  }
+  // into digit order in shared memory
 #pragma unroll
-    for (int it = 0; it < RS_ITEMS; it++) {
-      const uint32_t j = it * RS_THREADS + threadIdx.x;
-      if (j < nblk) {
-        const uint32_t k = sm.keys[j];
-        const uint32_t dst = sm.gdelta[(k >> shift) & 255u] + j;
-        keys_out[dst] = k;
-        vals_out[dst] = sm.vals[j];
-      }
+  for (int it = 0; it < RS_ITEMS; it++) {
+    const uint32_t idx = base + it * 32 + lane;
+    if (idx < n) {
+      const uint32_t d = (key[it] >> shift) & 255u;
+      const uint32_t lpos = sm.lbase[d] + sm.cnt[warp][d] + rank[it];
+      sm.keys[lpos] = key[it];
+      sm.vals[lpos] = val[it];
     }
-    __syncthreads();  // shared memory is reused by the next tile
+  }
+  __syncthreads();
+  const uint32_t nblk = min((uint32_t)RS_TILE, n - tile * (uint32_t)RS_TILE);
+#pragma unroll
+  for (int it = 0; it < RS_ITEMS; it++) {
+    const uint32_t j = it * RS_THREADS + threadIdx.x;
+    if (j < nblk) {
+      const uint32_t k = sm.keys[j];
+      const uint32_t dst = sm.gdelta[(k >> shift) & 255u] + j;
+      keys_out[dst] = k;
+      vals_out[dst] = sm.vals[j];
+    }
   }
 }
 
 // Depth keys: fp32 bits of depth (positive floats order as unsigned ints); culled Gaussians last.
-// Also R = sum of tiles_touched and the number of visible Gaussians.
+// Also R = sum of tiles_touched, the number of visible Gaussians, and the digit histograms of all four
+// radix passes (they do not depend on the order of the keys, so one read of the keys gives all of them).
 __global__ void __launch_bounds__(256) depth_keys_kernel(int64_t N, const float* __restrict__ depths,
                                                          const uint32_t* __restrict__ tiles_touched,
                                                          uint32_t* __restrict__ keys, SortCtl* __restrict__ ctl) {
   __shared__ unsigned long long s_sum[8];
   __shared__ uint32_t s_vis[8];
-  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  uint32_t tt = 0;
-  if (i < N) {
-    tt = tiles_touched[i];
-    keys[i] = tt ? __float_as_uint(depths[i]) : 0xffffffffu;
-  }
-  const uint32_t vis = __popc(__ballot_sync(0xffffffffu, tt != 0));
-  unsigned long long sum = tt;
+  __shared__ uint32_t hist[4][RS_BINS];
+  for (int j = threadIdx.x; j < 4 * RS_BINS; j += 256) (&hist[0][0])[j] = 0;
+  __syncthreads();
+  unsigned long long sum = 0;
+  uint32_t vis = 0;
+  for (int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x; i < N; i += (int64_t)gridDim.x * 256) {
+    const uint32_t tt = tiles_touched[i];
+    const uint32_t key = tt ? __float_as_uint(depths[i]) : 0xffffffffu;
+    keys[i] = key;
+    sum += tt;
+    vis += tt != 0;
 #pragma unroll
-  for (int o = 16; o >= 1; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+    for (int p = 0; p < 4; p++) atomicAdd(&hist[p][(key >> (8 * p)) & 255u], 1u);
+  }
+#pragma unroll
+  for (int o = 16; o >= 1; o >>= 1) {
+    sum += __shfl_xor_sync(0xffffffffu, sum, o);
+    vis += __shfl_xor_sync(0xffffffffu, vis, o);
+  }
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   if (lane == 0) { s_sum[warp] = sum; s_vis[warp] = vis; }
   __syncthreads();
@@ -232,10 +262,23 @@ __global__ void __launch_bounds__(256) depth_keys_kernel(int64_t N, const float*
     if (t) atomicAdd(&ctl->R, t);
     if (v) atomicAdd(&ctl->nvis, v);
   }
+  for (int j = threadIdx.x; j < 4 * RS_BINS; j += 256) {
+    const uint32_t c = (&hist[0][0])[j];
+    if (c) atomicAdd(&ctl->ghist[0][0] + j, c);
+  }
 }
 
-__global__ void ctl_finalize_kernel(SortCtl* __restrict__ ctl, unsigned long long capacity) {
-  ctl->overflow = (ctl->R > capacity || ctl->R >= (1ull << 32)) ? 1u : 0u;
+// Overflow flag; digit histograms -> exclusive digit bases (one block of 256 threads).
+__global__ void __launch_bounds__(RS_BINS) ctl_finalize_kernel(SortCtl* __restrict__ ctl, unsigned long long capacity) {
+  __shared__ uint32_t h[4][RS_BINS];
+  if (threadIdx.x == 0) ctl->overflow = (ctl->R > capacity || ctl->R >= (1ull << 32)) ? 1u : 0u;
+  for (int p = 0; p < 4; p++) h[p][threadIdx.x] = ctl->ghist[p][threadIdx.x];
+  __syncthreads();
+  for (int p = 0; p < 4; p++) {
+    uint32_t run = 0;
+    for (int d = 0; d < (int)threadIdx.x; d++) run += h[p][d];
+    ctl->ghist[p][threadIdx.x] = run;
+  }
 }
 
 // ---------------------------------------------------------------- exclusive scan of a uint32 table
@@ -589,7 +632,7 @@ __global__ void __launch_bounds__(256) tile_order_kernel(const uint32_t* __restr
 }
 
 struct Layout {
-  size_t ctl, keysA, valsA, keysB, valsB, table_n, sums, prect, table_r, row_start, chunk_base, row_rec, table_c, total;
+  size_t ctl, keysA, valsA, keysB, valsB, status, sums, prect, table_r, row_start, chunk_base, row_rec, table_c, total;
   int nblk_sort;          // blocks of a radix pass over N
   uint32_t n_chunks_r;    // warps of the row expansion
   uint32_t max_chunks_c;  // upper bound of the warps of the column expansion
@@ -605,7 +648,7 @@ Layout make_layout(int64_t N, int gw, int gh, uint64_t Rcap) {
   L.n_chunks_r = (uint32_t)((n + XP_CHUNK - 1) / XP_CHUNK);
   L.max_chunks_c = (uint32_t)(r / XP_CHUNK + (size_t)gh);
   const size_t tn = (size_t)RS_BINS * L.nblk_sort, tr = (size_t)gh * L.n_chunks_r, tc = (size_t)gw * L.max_chunks_c;
-  size_t tmax = tn > tr ? tn : tr;
+  size_t tmax = tr;
   if (tc > tmax) tmax = tc;
   L.max_scan_blocks = (uint32_t)((tmax + SCAN_BLK - 1) / SCAN_BLK + 1);
   size_t o = 0;
@@ -614,7 +657,7 @@ Layout make_layout(int64_t N, int gw, int gh, uint64_t Rcap) {
   L.valsA = o; o = align256(o + 4 * n);
   L.keysB = o; o = align256(o + 4 * n);
   L.valsB = o; o = align256(o + 4 * n);
-  L.table_n = o; o = align256(o + 4 * (tn + 1));
+  L.status = o; o = align256(o + 8 * 4 * tn);  // look-back status words of the four radix passes
   L.sums = o; o = align256(o + 4 * (size_t)L.max_scan_blocks);
   L.prect = o; o = align256(o + 8 * n);
   L.table_r = o; o = align256(o + 4 * (tr + 1));
@@ -679,7 +722,8 @@ extern "C" int mg_bin_sort(const mg_camera* cam, int64_t N, const float* depths,
   SortCtl* ctl = (SortCtl*)(ws + L.ctl);
   uint32_t *keysA = (uint32_t*)(ws + L.keysA), *valsA = (uint32_t*)(ws + L.valsA);
   uint32_t *keysB = (uint32_t*)(ws + L.keysB), *valsB = (uint32_t*)(ws + L.valsB);
-  uint32_t *table_n = (uint32_t*)(ws + L.table_n), *sums = (uint32_t*)(ws + L.sums);
+  unsigned long long* status = (unsigned long long*)(ws + L.status);
+  uint32_t* sums = (uint32_t*)(ws + L.sums);
   uint2* prect = (uint2*)(ws + L.prect);
   uint32_t* table_r = (uint32_t*)(ws + L.table_r);
   uint32_t *row_start = (uint32_t*)(ws + L.row_start), *chunk_base = (uint32_t*)(ws + L.chunk_base);
@@ -697,30 +741,27 @@ extern "C" int mg_bin_sort(const mg_camera* cam, int64_t N, const float* depths,
     return MG_OK;
   }
 
-  // S1: depth order of the N Gaussians (culled ones last), R, nvis, overflow flag
-  // radix passes run as persistent grids (one wave of resident blocks looping over the logical tiles)
-  static int rs_grid_count = 0, rs_grid_scatter = 0;
-  if (rs_grid_scatter == 0) {
-    MG_CHECK_CUDA(cudaFuncSetAttribute(radix_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(RadixSmem)));
-    int dev = 0, sms = 0, occ_c = 0, occ_s = 0;
+  // S1: depth order of the N Gaussians (culled ones last), R, nvis, overflow flag, digit histograms
+  static int dk_grid = 0;
+  if (dk_grid == 0) {
+    MG_CHECK_CUDA(cudaFuncSetAttribute(radix_onesweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(RadixSmem)));
+    int dev = 0, sms = 0;
     MG_CHECK_CUDA(cudaGetDevice(&dev));
     MG_CHECK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    MG_CHECK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_c, radix_count_kernel, RS_THREADS, 0));
-    MG_CHECK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_s, radix_scatter_kernel, RS_THREADS, sizeof(RadixSmem)));
-    rs_grid_count = sms * (occ_c > 0 ? occ_c : 1);
-    rs_grid_scatter = sms * (occ_s > 0 ? occ_s : 1);
+    dk_grid = sms * 8;
   }
-  const int grid_c = L.nblk_sort < rs_grid_count ? L.nblk_sort : rs_grid_count;
-  const int grid_s = L.nblk_sort < rs_grid_scatter ? L.nblk_sort : rs_grid_scatter;
-  depth_keys_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(N, depths, tiles_touched, keysA, ctl);
-  ctl_finalize_kernel<<<1, 1, 0, st>>>(ctl, (unsigned long long)R_capacity);
+  MG_CHECK_CUDA(cudaMemsetAsync(status, 0, sizeof(unsigned long long) * 4 * (size_t)L.nblk_sort * RS_BINS, st));
+  {
+    const int64_t want = (N + 255) / 256;
+    depth_keys_kernel<<<(unsigned)(want < dk_grid ? want : dk_grid), 256, 0, st>>>(N, depths, tiles_touched, keysA, ctl);
+  }
+  ctl_finalize_kernel<<<1, RS_BINS, 0, st>>>(ctl, (unsigned long long)R_capacity);
   MG_CHECK_LAUNCH();
   {
     uint32_t *ki = keysA, *vi = nullptr, *ko = keysB, *vo = valsB;
     for (int pass = 0; pass < 4; pass++) {
-      radix_count_kernel<<<grid_c, RS_THREADS, 0, st>>>(ki, (uint32_t)N, 8 * pass, table_n, L.nblk_sort);
-      if (int rc = scan_table(table_n, (uint32_t)(RS_BINS * L.nblk_sort), nullptr, (uint32_t)(RS_BINS * L.nblk_sort), sums, st)) return rc;
-      radix_scatter_kernel<<<grid_s, RS_THREADS, sizeof(RadixSmem), st>>>(ki, vi, ko, vo, (uint32_t)N, 8 * pass, table_n, L.nblk_sort);
+      radix_onesweep_kernel<<<L.nblk_sort, RS_THREADS, sizeof(RadixSmem), st>>>(
+          ki, vi, ko, vo, (uint32_t)N, pass, ctl, status + (size_t)pass * L.nblk_sort * RS_BINS);
       MG_CHECK_LAUNCH();
       ki = (pass & 1) ? keysA : keysB;
       vi = (pass & 1) ? valsA : valsB;
