@@ -1,5 +1,6 @@
-"""Parity at BASELINE.json's full size (configs[2]: 3 M Gaussians, 1297x840, SH degree 3) in the launch
-configuration bench.py times.  Projection, sort and projection-backward are compared in full; the two
+"""Parity at BASELINE.json's full sizes -- configs[2] (3 M Gaussians, 1297x840: the bench workload), configs[3]
+(2.8 M, 1264x832, indoor) and configs[4] (6 M, 1920x1080, keep-probability 0.9: the largest size and the
+longest tile lists), camera 0, SH degree 3 -- in the launch configuration bench.py times.  Projection, sort and projection-backward are compared in full; the two
 blend kernels on a seeded sample of tiles the oracle can walk in seconds (the other tiles' ranges are
 emptied for both sides, which leaves the sampled tiles' arithmetic untouched)."""
 import numpy as np
@@ -13,11 +14,13 @@ from paper_2412_20522_b200 import scenes
 pytestmark = pytest.mark.gpu
 
 
-@pytest.fixture(scope="module")
-def full(oracle):
-    sc = scenes.config3()
+@pytest.fixture(scope="module", params=[3, 4, 5])
+def full(request, oracle):
+    sc = scenes.make(request.param)
     fr, g, m, gimg = pu.run_gpu(sc)
-    return sc, fr, g, m, gimg
+    yield sc, fr, g, m, gimg
+    del fr, g, m, gimg
+    torch.cuda.empty_cache()
 
 
 def test_full_size_projection_and_sort(full, oracle):
@@ -26,7 +29,7 @@ def test_full_size_projection_and_sort(full, oracle):
     s1 = pu.check_preprocess(fr, sc, cam, max_flag_frac=0.02)
     ids, ranges = pu.check_bin_sort(fr, cam)
     assert fr.R > 10_000_000
-    print("cfg3 preprocess", s1, "R", fr.R)
+    print(sc.name, "preprocess", s1, "R", fr.R)
 
 
 def test_full_size_blend_on_sampled_tiles(full, oracle):
@@ -43,7 +46,7 @@ def test_full_size_blend_on_sampled_tiles(full, oracle):
     ranges_s[tiles] = ranges_full[tiles]
     ids = pu.u32(fr.sorted_ids)[: fr.R]
     ref, s3 = pu.check_render_fwd(fr, cam, sc.masks, ids, ranges_s, tiles=tiles, max_flag_frac=0.05)
-    print("cfg3 fwd sampled tiles", len(tiles), s3)
+    print(sc.name, "fwd sampled tiles", len(tiles), s3)
     # backward restricted to the same tiles on both sides
     keep_ranges = fr.tile_ranges.clone()
     fr.tile_ranges.copy_(torch.from_numpy(ranges_s.view(np.int32)).cuda())
@@ -51,7 +54,7 @@ def test_full_size_blend_on_sampled_tiles(full, oracle):
     torch.cuda.synchronize()
     try:
         _, s4 = pu.check_render_bwd(fr, cam, sc.N, sc.masks, ids, ranges_s, sc.dL_dimage(), max_flag_frac=0.3)
-        print("cfg3 bwd sampled tiles", {k: round(v, 4) for k, v in s4.items()})
+        print(sc.name, "bwd sampled tiles", {k: round(v, 4) for k, v in s4.items()})
     finally:
         fr.tile_ranges.copy_(keep_ranges)
         fr.render_bwd(m, gimg)
@@ -64,7 +67,7 @@ def test_full_size_projection_backward(full, oracle):
     ref5, s5 = pu.check_preprocess_bwd(fr, sc, cam)
     for k, v in s5.items():
         assert v <= 2e-4, f"{k}: relative 2-norm error {v:.2e}"
-    print("cfg3 preprocess_bwd", s5)
+    print(sc.name, "preprocess_bwd", s5)
 
 
 def test_full_size_invariants(full):
