@@ -17,7 +17,7 @@
 //
 // S2 and S3 are the same primitive, a STABLE INTERVAL EXPANSION: items in sequence order, each with
 // an interval of bins, are appended to every bin of their interval, order preserved.  A warp takes
-// a chunk of 512 consecutive items, 32 at a time.  Counting: a difference array per chunk in shared
+// a chunk of 128 consecutive items, 32 at a time.  Counting: a difference array per chunk in shared
 // memory (two atomics per item), scanned over the bins at the end.  Per chunk and bin the counts go
 // to a table, an exclusive scan of the table (bin-major, chunk-minor) gives every (bin, chunk) its
 // write position, and a second sweep emits: lane k turns its interval into a row of a 32 x 32-bin bit
@@ -44,7 +44,10 @@ constexpr int RS_WARPS = RS_THREADS / 32;
 constexpr int RS_TILE = RS_THREADS * RS_ITEMS;  // 4096 elements per block: 41 KB of shared memory, 5 blocks per SM
 constexpr int RS_BINS = 256;
 
-constexpr int XP_CHUNK = 512;   // items per warp in the expansion sweeps
+#ifndef XP_CHUNK_
+#define XP_CHUNK_ 128
+#endif
+constexpr int XP_CHUNK = XP_CHUNK_;   // items per warp in the expansion sweeps
 constexpr int XP_MAX_WARPS = 8; // warps per block in the expansion sweeps
 constexpr int SCAN_THREADS = 1024;
 constexpr int SCAN_ITEMS = 4;
