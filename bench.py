@@ -31,6 +31,9 @@ if ROOT not in sys.path:
 FLOP_PAIR = 13        # per pair evaluation: 2 sub, 6 quadratic form, mul, min, 2 compares (+1 MUFU not counted)
 FLOP_BLEND_FWD = 11   # per blend, forward
 FLOP_BLEND_BWD = 59   # per blend, backward (49 + 10 adds of the per-entry reduction)
+# dram__bytes_read.sum + dram__bytes_write.sum per launch at config 3, from the `ncu --set full` capture summarised
+# in profiles/r01z_final.md (the report itself is not committed); null for other configs
+NCU_TRAFFIC_BYTES = {3: {"render_bwd": 856.3e6 + 115.2e6, "render_fwd": 279.7e6 + 19.8e6}}
 # kernels of libmg launched per step (memsets and copies not counted): bin_sort = depth keys + ctl + 4 single-kernel
 # radix passes + row expansion (count, 2 scan, plan, emit) + column expansion (count, 2 scan, emit, ranges, tile order)
 KERNELS_PER_STEP = {"preprocess": 1, "bin_sort": 2 + 4 + 5 + 6, "render_fwd": 1, "render_bwd": 1,
@@ -298,7 +301,9 @@ def main():
             flops = wc["fwd_pair_evals"] * FLOP_PAIR + wc["fwd_blends"] * FLOP_BLEND_FWD
         ach = flops / (per_call[dom] * 1e-3) / 1e12
         roofline = {"kernel": dom + "_kernel", "bound": "alu", "achieved": ach, "peak": fp32_peak, "unit": "TFLOP/s",
-                    "frac": ach / fp32_peak, "traffic": None, "share_of_step": per_call[dom] / sum(per_call.values()),
+                    "frac": ach / fp32_peak,
+                    "traffic": NCU_TRAFFIC_BYTES.get(args.config, {}).get(dom), "traffic_unit": "bytes per launch (ncu, profiles/r01z_final.md)",
+                    "flop_per_launch": flops, "share_of_step": per_call[dom] / sum(per_call.values()),
                     "peak_source": f"derived 148 SM x 128 lanes x 2 x {sm_max:.0f} MHz (no FP32 entry in MEASURED_PEAKS.json)"}
 
     cpu = None
