@@ -98,7 +98,7 @@ def oracle_sample(cfg, n_tiles_target=None, seed=0):
     gw, gh = orc.grid(cam)
     ntiles = gw * gh
     if n_tiles_target is None:
-        n_tiles_target = max(96, ntiles // 4)  # ~10-30 s of CPU work at config 3
+        n_tiles_target = ntiles if ntiles <= 5000 else ntiles // 2  # config 3: the whole frame, ~10-20 s of CPU work
     stride = max(1, ntiles // n_tiles_target)
     sel = np.zeros(ntiles, np.uint8)
     sel[seed % stride::stride] = 1
@@ -119,7 +119,8 @@ def oracle_sample(cfg, n_tiles_target=None, seed=0):
     blends = fwd["blends"] + rb["blends"]
     # per-Gaussian steps run on the whole scene; charge the sample its share of them
     seconds = (t3 - t2) + (t4 - t3) + (t2 - t1) + frac * ((t1 - t0) + (t5 - t4))
-    info = (f"{int(sel.sum())} of {ntiles} tiles (every {stride}th) of config {cfg}: oracle bin_sort+render_fwd+render_bwd "
+    which = "the whole frame" if stride == 1 else f"every {stride}th tile"
+    info = (f"{int(sel.sum())} of {ntiles} tiles ({which}) of config {cfg}: oracle bin_sort+render_fwd+render_bwd "
             f"on those tiles ({t2 - t1:.1f}+{t3 - t2:.1f}+{t4 - t3:.1f} s) + {frac:.4f} x (preprocess {t1 - t0:.1f} s + "
             f"preprocess_bwd {t5 - t4:.1f} s)")
     return blends, seconds, info
