@@ -67,13 +67,21 @@ class ClockSampler:
         for line in self.proc.stdout:
             self.rows.append(line.strip())
 
+    def mark(self, timeout=5.0):
+        """Wait until nvidia-smi has started emitting, then remember where the timed region begins."""
+        t0 = time.time()
+        while self.proc is not None and not self.rows and time.time() - t0 < timeout:
+            time.sleep(0.02)
+        self.first = len(self.rows)
+
     def stop(self):
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         self.proc.terminate()
         self.t.join(timeout=2)
         sm, mx, reasons = [], [], set()
-        for r in self.rows:
+        rows = self.rows[getattr(self, "first", 0):] or self.rows[-1:]
+        for r in rows:
             f = [x.strip() for x in r.split(",")]
             if len(f) < 7:
                 continue
@@ -232,6 +240,8 @@ def main():
     names = ["preprocess", "bin_sort", "render_fwd", "render_bwd", "preprocess_bwd"]
     ev = [[torch.cuda.Event(enable_timing=True) for _ in range(6)] for _ in range(args.steps)]
     sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        sampler.mark()
     barrier()
     for s in range(args.steps):
         e = ev[s]

@@ -131,11 +131,11 @@ __global__ void __launch_bounds__(RN_THREADS, RN_BWD_MINB) render_bwd_kernel(
 
   // where this lane's reduced sum goes
   const int slot = slot_of_lane(lane);
-  float* tgt_base = nullptr;
-  int tgt_stride = 0, tgt_off = 0;
+  float* tgt_ptr = nullptr;  // element 0 of this lane's component; Gaussian id lives tgt_stride floats further on
+  uint32_t tgt_stride = 0;
 #pragma unroll
   for (int s = 0; s < 10; s++)
-    if (slot == s) { tgt_base = tg.base[s]; tgt_stride = tg.stride[s]; tgt_off = tg.offset[s]; }
+    if (slot == s) { tgt_ptr = tg.base[s] + tg.offset[s]; tgt_stride = (uint32_t)tg.stride[s]; }
   float* const dmask = tg.base[9];
 
   const int n = (int)wmax;  // entries at positions > wmax are never visited by this warp
@@ -252,7 +252,7 @@ __global__ void __launch_bounds__(RN_THREADS, RN_BWD_MINB) render_bwd_kernel(
       const float total = transpose_reduce10(v, lane);
       if (slot >= 0 && total != 0.f) {
         const uint32_t id = ids_sh[jj];
-        atomicAdd(tgt_base + (size_t)id * tgt_stride + tgt_off, total);
+        atomicAdd(tgt_ptr + (size_t)id * tgt_stride, total);
       }
     }
   }
