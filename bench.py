@@ -146,6 +146,57 @@ def max_over_ranks(value, world, device):
     return float(t.item())
 
 
+def bench_mask_head(sc, g, hbm_gbs, reps=20):
+    """SURVEY.md 8(f) row f1, measured like the hot path (CUDA events, warm, inputs resident): the mask head at the
+    bench workload's N.  Algorithmic bytes per Gaussian: sample 24 (2 scores + 2 uniforms in, mask + soft out),
+    loss 12, backward 16, prune rule 89 (10 draws), compaction 4 x 61 floats in + the kept rows out."""
+    import torch
+
+    from paper_2412_20522_b200 import binding as mg
+    from paper_2412_20522_b200 import scenes
+
+    n = sc.N
+    scores_np, u_np, u10_np, gm_np = scenes.mask_head_inputs(n)
+    t = lambda a: torch.from_numpy(a).cuda()
+    scores, u, u10, dmask = t(scores_np), t(u_np), t(u10_np), t(gm_np)
+    masks, soft = torch.empty(n, device="cuda"), torch.empty(n, device="cuda")
+    dscores = torch.empty(n, 2, device="cuda")
+    stats = torch.zeros(3, dtype=torch.float64, device="cuda")
+    keep = torch.empty(n, dtype=torch.uint8, device="cuda")
+    src = [g["means"], g["log_scales"], g["quats"], g["opacity_logits"], g["sh"], scores]
+    dst = [torch.empty_like(x) for x in src]
+    ws = torch.empty(mg.mg_compact_workspace_bytes(n), dtype=torch.uint8, device="cuda")
+    n_out = torch.zeros(1, dtype=torch.int64).pin_memory()
+    calls = {
+        "mask_sample": lambda: mg.mg_mask_sample(scores, u, 1.0, masks, soft),
+        "mask_loss": lambda: mg.mg_mask_loss(masks, 0.1, dmask, stats),
+        "mask_sample_bwd": lambda: mg.mg_mask_sample_bwd(soft, dmask, 1.0, dscores),
+        "mask_prune_keep": lambda: mg.mg_mask_prune_keep(scores, u10, keep),
+        "compact": lambda: mg.mg_compact(keep, src, dst, ws, n_out),
+    }
+    out = {}
+    for name, fn in calls.items():
+        for _ in range(3):
+            fn()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(reps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        out[name] = e0.elapsed_time(e1) / reps
+    kept = int(n_out[0])
+    row = sum(x.numel() // n for x in src) * 4
+    nbytes = {"mask_sample": 24 * n, "mask_loss": 12 * n, "mask_sample_bwd": 16 * n, "mask_prune_keep": 89 * n,
+              "compact": n * (row + 1 + 4) + kept * row}
+    return {"N": n, "kept_by_prune_rule": kept,
+            "ms": {k: round(v, 4) for k, v in out.items()},
+            "gb_per_s": {k: round(nbytes[k] / (out[k] * 1e-3) / 1e9, 1) for k in out},
+            "frac_of_hbm_peak": {k: round(nbytes[k] / (out[k] * 1e-3) / 1e9 / hbm_gbs, 3) for k in out},
+            "peak_gb_per_s": hbm_gbs}
+
+
 def n_threads():
     try:
         return len(os.sched_getaffinity(0))
@@ -370,6 +421,11 @@ def main():
                     "flop_per_launch": flops, "share_of_step": per_call[dom] / sum(per_call.values()),
                     "peak_source": f"derived 148 SM x 128 lanes x 2 x {sm_max:.0f} MHz (no FP32 entry in MEASURED_PEAKS.json)"}
 
+    hbm_gbs = 6540.8
+    if os.path.exists(peaks_path):
+        hbm_gbs = float(json.load(open(peaks_path)).get("hbm_gbs", hbm_gbs))
+    next_rows = {"mask_head": bench_mask_head(sc, g, hbm_gbs)} if world == 1 else None
+
     cpu = None
     if not args.no_cpu_baseline:
         b, sec, info = oracle_sample(args.config)
@@ -389,7 +445,7 @@ def main():
             "e2e": {"value": e2e_value, "unit": "blends/s", "ms_per_step": e2e_ms, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "how": "pinned host buffers; H2D of all inputs and D2H of image + all gradients every step, software-pipelined over 3 streams and 2 buffer sets",
                     "ms_per_step_unpipelined": e2e_serial_ms},
-            "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu}
+            "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu, "next_rows": next_rows}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

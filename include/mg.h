@@ -138,6 +138,37 @@ int mg_preprocess_bwd(const mg_camera* cam, int64_t N, const float* means, const
                       const float* dL_dopacity, const float* dL_drgb, float* dL_dmeans, float* dL_dlog_scales,
                       float* dL_dquats, float* dL_dopacity_logits, float* dL_dsh, void* stream);
 
+/* ---- The mask head around the rasterizer.  Random numbers are INPUTS: the library draws none.
+ *
+ * mg_mask_sample (sec. 3.3: "we assign 2 learnable mask scores for each Gaussian, and apply Gumbel-Softmax
+ * to sample one differentiable category out of the 2 scores, denoted M_i in {0,1}").  scores[N][2], uniforms[N][2] in
+ * (0,1); g = -log(-log u); d = (s_1 + g_1) - (s_0 + g_0); masks[i] = 1 if d > 0 else 0 (category 1 = present, a tie
+ * gives 0); soft[i] (may be NULL) = softmax((s + g) / tau)_1 = sigmoid(d / tau), kept for the backward pass.
+ * tau > 0 is not stated in the paper (reading 22). */
+int mg_mask_sample(int64_t N, const float* scores, const float* uniforms, float tau, float* masks, float* soft,
+                   void* stream);
+
+/* Straight-through gradient of the hard sample (reading 23): dL_dscores[i] = (-t, t), t = dL_dmask[i] y (1 - y) / tau,
+ * y = soft[i].  dL_dscores[N][2] is overwritten. */
+int mg_mask_sample_bwd(int64_t N, const float* soft, const float* dL_dmask, float tau, float* dL_dscores, void* stream);
+
+/* Eq. 7-8: L_m = (1/N sum M_i)^2, L = L_render + lambda_m L_m.  stats (DEVICE, 3 doubles, overwritten):
+ * stats[0] = sum M, stats[1] = lambda_m L_m, stats[2] = mean M.  If dL_dmask is not NULL, lambda_m * 2 * mean / N is
+ * ADDED to every element (it already holds dL_render/dM from mg_render_bwd). */
+int mg_mask_loss(int64_t N, const float* masks, float lambda_m, float* dL_dmask, double* stats, void* stream);
+
+/* "we sample each Gaussian 10 times and remove those that are never sampled".  uniforms[n_draws][N][2];
+ * keep[i] = 1 iff M_i = 1 in at least one draw. */
+int mg_mask_prune_keep(int64_t N, int32_t n_draws, const float* scores, const float* uniforms, uint8_t* keep, void* stream);
+
+/* Stable compaction by keep[N]: for each of the n_arrays (<= 16) arrays of row_floats[a] floats per Gaussian, the rows
+ * of the kept Gaussians are copied, in order, to dst[a] (capacity N rows; src and dst must not overlap).  src, dst and
+ * row_floats are HOST arrays (of device pointers / ints).  *N_out_host = number kept, written asynchronously.
+ * workspace: mg_compact_workspace_bytes(N) bytes of device memory, 256-byte aligned. */
+size_t mg_compact_workspace_bytes(int64_t N);
+int mg_compact(int64_t N, const uint8_t* keep, int32_t n_arrays, const float* const* src, float* const* dst,
+               const int32_t* row_floats, void* workspace, size_t workspace_bytes, uint64_t* N_out_host, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

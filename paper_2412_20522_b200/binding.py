@@ -33,7 +33,8 @@ class mg_camera(C.Structure):
 
 
 EXPORTS = ["mg_last_error_string", "mg_version", "mg_workspace_bytes", "mg_preprocess", "mg_bin_sort",
-           "mg_render_fwd", "mg_render_bwd", "mg_preprocess_bwd"]
+           "mg_render_fwd", "mg_render_bwd", "mg_preprocess_bwd", "mg_mask_sample", "mg_mask_sample_bwd", "mg_mask_loss",
+           "mg_mask_prune_keep", "mg_compact_workspace_bytes", "mg_compact"]
 
 
 def lib():
@@ -47,8 +48,11 @@ def lib():
         L.mg_last_error_string.restype = C.c_char_p
         L.mg_workspace_bytes.restype = C.c_size_t
         L.mg_workspace_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int32, C.c_uint64]
+        L.mg_compact_workspace_bytes.restype = C.c_size_t
+        L.mg_compact_workspace_bytes.argtypes = [C.c_int64]
         for name in EXPORTS[3:]:
-            getattr(L, name).restype = C.c_int
+            if name != "mg_compact_workspace_bytes":
+                getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
 
@@ -144,6 +148,47 @@ def mg_preprocess_bwd(cam: mg_camera, means, log_scales, quats, opacity_logits, 
                                    _ptr(dL_dopacity, F32), _ptr(dL_drgb, F32), _ptr(dL_dmeans, F32),
                                    _ptr(dL_dlog_scales, F32), _ptr(dL_dquats, F32), _ptr(dL_dopacity_logits, F32),
                                    _ptr(dL_dsh, F32), _stream()))
+
+
+def mg_mask_sample(scores, uniforms, tau, masks, soft=None):
+    N = scores.shape[0]
+    _check(lib().mg_mask_sample(C.c_int64(N), _ptr(scores, F32), _ptr(uniforms, F32), C.c_float(tau), _ptr(masks, F32),
+                                _ptr(soft, F32), _stream()))
+
+
+def mg_mask_sample_bwd(soft, dL_dmask, tau, dL_dscores):
+    N = soft.shape[0]
+    _check(lib().mg_mask_sample_bwd(C.c_int64(N), _ptr(soft, F32), _ptr(dL_dmask, F32), C.c_float(tau),
+                                    _ptr(dL_dscores, F32), _stream()))
+
+
+def mg_mask_loss(masks, lambda_m, dL_dmask, stats):
+    N = masks.shape[0]
+    _check(lib().mg_mask_loss(C.c_int64(N), _ptr(masks, F32), C.c_float(lambda_m), _ptr(dL_dmask, F32),
+                              _ptr(stats, torch.float64), _stream()))
+
+
+def mg_mask_prune_keep(scores, uniforms, keep):
+    N, S = scores.shape[0], uniforms.shape[0]
+    _check(lib().mg_mask_prune_keep(C.c_int64(N), C.c_int32(S), _ptr(scores, F32), _ptr(uniforms, F32), _ptr(keep, U8),
+                                    _stream()))
+
+
+def mg_compact_workspace_bytes(N) -> int:
+    return int(lib().mg_compact_workspace_bytes(int(N)))
+
+
+def mg_compact(keep, src, dst, workspace, N_out_host=None):
+    """src / dst: lists of contiguous fp32 tensors with N rows each (row size = numel / N)."""
+    N = keep.shape[0]
+    n = len(src)
+    srcp = (C.c_void_p * n)(*[t.data_ptr() for t in src])
+    dstp = (C.c_void_p * n)(*[t.data_ptr() for t in dst])
+    rows = (C.c_int32 * n)(*[(t.numel() // N if N else 1) for t in src])
+    for t in list(src) + list(dst):
+        assert t.is_contiguous() and t.dtype == F32 and t.device.type == "cuda"
+    _check(lib().mg_compact(C.c_int64(N), _ptr(keep, U8), C.c_int32(n), srcp, dstp, rows, _ptr(workspace, U8),
+                            C.c_size_t(workspace.numel()), _ptr(N_out_host, torch.int64, "cpu"), _stream()))
 
 
 class Frame:

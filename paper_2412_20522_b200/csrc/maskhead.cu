@@ -1,0 +1,225 @@
+// maskhead.cu -- the mask head around the rasterizer.
+//   mg_mask_sample      Gumbel-Softmax over 2 scores per Gaussian -> hard mask M_i in {0,1} + soft sample
+//   mg_mask_sample_bwd  straight-through gradient of the sample to the two scores
+//   mg_mask_loss        lambda_m L_m = lambda_m (mean M)^2 (Eq. 7-8) and its gradient, added to dL/dM
+//   mg_mask_prune_keep  "sample each Gaussian 10 times and remove those that are never sampled"
+//   mg_compact          stable compaction of the attribute arrays by the keep flags
+// All elementwise and HBM-bound: one pass over the data, coalesced, no intermediate arrays.  Random numbers are
+// inputs (uniforms in (0,1)); the library draws none.
+#include "mg_common.cuh"
+
+namespace {
+
+constexpr int MH_THREADS = 256;
+
+// d = (s_1 + g_1) - (s_0 + g_0) with g = -log(-log u): the hard sample is d > 0, the soft one sigmoid(d / tau).
+__device__ __forceinline__ float perturbed_gap(float2 s, float2 u) {
+  const float g0 = -logf(-logf(u.x)), g1 = -logf(-logf(u.y));
+  return (s.y + g1) - (s.x + g0);
+}
+
+__global__ void __launch_bounds__(MH_THREADS) mask_sample_kernel(int64_t N, const float2* __restrict__ scores,
+                                                                 const float2* __restrict__ uniforms, float inv_tau,
+                                                                 float* __restrict__ masks, float* __restrict__ soft) {
+  const int64_t i = (int64_t)blockIdx.x * MH_THREADS + threadIdx.x;
+  if (i >= N) return;
+  const float d = perturbed_gap(scores[i], uniforms[i]);
+  masks[i] = d > 0.f ? 1.f : 0.f;
+  if (soft) soft[i] = 1.f / (1.f + expf(-d * inv_tau));
+}
+
+__global__ void __launch_bounds__(MH_THREADS) mask_sample_bwd_kernel(int64_t N, const float* __restrict__ soft,
+                                                                     const float* __restrict__ dL_dmask, float inv_tau,
+                                                                     float2* __restrict__ dL_dscores) {
+  const int64_t i = (int64_t)blockIdx.x * MH_THREADS + threadIdx.x;
+  if (i >= N) return;
+  const float y = soft[i];
+  const float t = dL_dmask[i] * y * (1.f - y) * inv_tau;
+  dL_dscores[i] = make_float2(-t, t);
+}
+
+// stats[0] += sum of masks (double: exact for 0/1 masks whatever the order of the atomics)
+__global__ void __launch_bounds__(MH_THREADS) mask_sum_kernel(int64_t N, const float* __restrict__ masks, double* __restrict__ stats) {
+  __shared__ double part[MH_THREADS / 32];
+  double s = 0.0;
+  for (int64_t i = (int64_t)blockIdx.x * MH_THREADS + threadIdx.x; i < N; i += (int64_t)gridDim.x * MH_THREADS) s += (double)masks[i];
+#pragma unroll
+  for (int o = 16; o >= 1; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+  if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double t = 0.0;
+#pragma unroll
+    for (int w = 0; w < MH_THREADS / 32; w++) t += part[w];
+    if (t != 0.0) atomicAdd(&stats[0], t);
+  }
+}
+
+// stats[1] = lambda_m (mean M)^2, stats[2] = mean M; dL_dmask[i] += lambda_m 2 mean / N
+__global__ void __launch_bounds__(MH_THREADS) mask_loss_apply_kernel(int64_t N, double lambda_m, double* __restrict__ stats,
+                                                                     float* __restrict__ dL_dmask) {
+  const double mean = stats[0] / (double)N;
+  const int64_t i = (int64_t)blockIdx.x * MH_THREADS + threadIdx.x;
+  if (i == 0) { stats[1] = lambda_m * mean * mean; stats[2] = mean; }
+  if (dL_dmask && i < N) dL_dmask[i] += (float)(lambda_m * 2.0 * mean / (double)N);
+}
+
+__global__ void __launch_bounds__(MH_THREADS) mask_prune_kernel(int64_t N, int S, const float2* __restrict__ scores,
+                                                                const float2* __restrict__ uniforms, uint8_t* __restrict__ keep) {
+  const int64_t i = (int64_t)blockIdx.x * MH_THREADS + threadIdx.x;
+  if (i >= N) return;
+  const float2 s = scores[i];
+  bool k = false;
+  for (int d = 0; d < S; d++) k = k || perturbed_gap(s, uniforms[(int64_t)d * N + i]) > 0.f;
+  keep[i] = k ? 1 : 0;
+}
+
+// ---- compaction: block counts -> scan of the block counts (one block) -> positions -> row copies
+constexpr int CP_BLOCK = 1024;
+
+__global__ void __launch_bounds__(CP_BLOCK) compact_count_kernel(int64_t N, const uint8_t* __restrict__ keep, uint32_t* __restrict__ block_counts) {
+  const int64_t i = (int64_t)blockIdx.x * CP_BLOCK + threadIdx.x;
+  const int c = __syncthreads_count(i < N && keep[i] != 0);
+  if (threadIdx.x == 0) block_counts[blockIdx.x] = (uint32_t)c;
+}
+
+__global__ void __launch_bounds__(1024) compact_scan_kernel(uint32_t* __restrict__ block_counts, int nblk, unsigned long long* __restrict__ total) {
+  __shared__ uint32_t part[1024];
+  const int per = (nblk + 1023) / 1024;
+  const int b = threadIdx.x * per, e = min(nblk, b + per);
+  uint32_t s = 0;
+  for (int j = b; j < e; j++) s += block_counts[j];
+  part[threadIdx.x] = s;
+  __syncthreads();
+  for (int o = 1; o < 1024; o <<= 1) {
+    const uint32_t v = threadIdx.x >= o ? part[threadIdx.x - o] : 0;
+    __syncthreads();
+    part[threadIdx.x] += v;
+    __syncthreads();
+  }
+  uint32_t run = part[threadIdx.x] - s;
+  for (int j = b; j < e; j++) { const uint32_t v = block_counts[j]; block_counts[j] = run; run += v; }
+  if (threadIdx.x == 1023) *total = part[1023];
+}
+
+__global__ void __launch_bounds__(CP_BLOCK) compact_pos_kernel(int64_t N, const uint8_t* __restrict__ keep,
+                                                               const uint32_t* __restrict__ block_offsets, uint32_t* __restrict__ pos) {
+  __shared__ uint32_t wsum[CP_BLOCK / 32];
+  const int64_t i = (int64_t)blockIdx.x * CP_BLOCK + threadIdx.x;
+  const bool k = i < N && keep[i] != 0;
+  const uint32_t ballot = __ballot_sync(0xffffffffu, k);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (lane == 0) wsum[warp] = __popc(ballot);
+  __syncthreads();
+  uint32_t woff = 0;
+  for (int w = 0; w < warp; w++) woff += wsum[w];
+  if (i < N) pos[i] = k ? block_offsets[blockIdx.x] + woff + __popc(ballot & ((1u << lane) - 1u)) : 0xffffffffu;
+}
+
+// One thread per input element (a float, or a float4 when the row size is a multiple of 4 floats): element e of an
+// array with r elements per row belongs to Gaussian e / r.  32-bit index arithmetic (the host checks the range).
+template <typename V>
+__global__ void __launch_bounds__(MH_THREADS) compact_rows_kernel(uint32_t n_elems, uint32_t r, const uint32_t* __restrict__ pos,
+                                                                  const V* __restrict__ src, V* __restrict__ dst) {
+  const uint32_t e = blockIdx.x * (uint32_t)MH_THREADS + threadIdx.x;
+  if (e >= n_elems) return;
+  const uint32_t i = e / r;
+  const uint32_t p = pos[i];
+  if (p != 0xffffffffu) dst[(size_t)p * r + (e - i * r)] = src[e];
+}
+
+inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+}  // namespace
+
+extern "C" int mg_mask_sample(int64_t N, const float* scores, const float* uniforms, float tau, float* masks, float* soft,
+                              void* stream) {
+  MG_REQUIRE(N >= 0 && N < (int64_t)1 << 31, "N must be in [0, 2^31)");
+  MG_REQUIRE(tau > 0.f, "tau must be positive");
+  if (N == 0) return MG_OK;
+  MG_REQUIRE(scores && uniforms && masks, "null array");
+  mask_sample_kernel<<<(unsigned)((N + MH_THREADS - 1) / MH_THREADS), MH_THREADS, 0, (cudaStream_t)stream>>>(
+      N, (const float2*)scores, (const float2*)uniforms, 1.f / tau, masks, soft);
+  MG_CHECK_LAUNCH();
+  return MG_OK;
+}
+
+extern "C" int mg_mask_sample_bwd(int64_t N, const float* soft, const float* dL_dmask, float tau, float* dL_dscores,
+                                  void* stream) {
+  MG_REQUIRE(N >= 0 && N < (int64_t)1 << 31, "N must be in [0, 2^31)");
+  MG_REQUIRE(tau > 0.f, "tau must be positive");
+  if (N == 0) return MG_OK;
+  MG_REQUIRE(soft && dL_dmask && dL_dscores, "null array");
+  mask_sample_bwd_kernel<<<(unsigned)((N + MH_THREADS - 1) / MH_THREADS), MH_THREADS, 0, (cudaStream_t)stream>>>(
+      N, soft, dL_dmask, 1.f / tau, (float2*)dL_dscores);
+  MG_CHECK_LAUNCH();
+  return MG_OK;
+}
+
+extern "C" int mg_mask_loss(int64_t N, const float* masks, float lambda_m, float* dL_dmask, double* stats, void* stream) {
+  MG_REQUIRE(N > 0 && N < (int64_t)1 << 31, "N must be in (0, 2^31)");
+  MG_REQUIRE(masks && stats, "null array");
+  cudaStream_t st = (cudaStream_t)stream;
+  MG_CHECK_CUDA(cudaMemsetAsync(stats, 0, 3 * sizeof(double), st));
+  const int64_t want = (N + MH_THREADS - 1) / MH_THREADS;
+  mask_sum_kernel<<<(unsigned)(want < 1184 ? want : 1184), MH_THREADS, 0, st>>>(N, masks, stats);
+  mask_loss_apply_kernel<<<(unsigned)want, MH_THREADS, 0, st>>>(N, (double)lambda_m, stats, dL_dmask);
+  MG_CHECK_LAUNCH();
+  return MG_OK;
+}
+
+extern "C" int mg_mask_prune_keep(int64_t N, int32_t n_draws, const float* scores, const float* uniforms, uint8_t* keep,
+                                  void* stream) {
+  MG_REQUIRE(N >= 0 && N < (int64_t)1 << 31, "N must be in [0, 2^31)");
+  MG_REQUIRE(n_draws >= 0, "n_draws must be >= 0");
+  if (N == 0) return MG_OK;
+  MG_REQUIRE(scores && keep && (uniforms || n_draws == 0), "null array");
+  mask_prune_kernel<<<(unsigned)((N + MH_THREADS - 1) / MH_THREADS), MH_THREADS, 0, (cudaStream_t)stream>>>(
+      N, n_draws, (const float2*)scores, (const float2*)uniforms, keep);
+  MG_CHECK_LAUNCH();
+  return MG_OK;
+}
+
+extern "C" size_t mg_compact_workspace_bytes(int64_t N) {
+  if (N < 0) return 0;
+  const size_t nblk = (size_t)((N + CP_BLOCK - 1) / CP_BLOCK);
+  return align256(8) + align256(4 * (nblk + 1)) + align256(4 * (size_t)N);
+}
+
+extern "C" int mg_compact(int64_t N, const uint8_t* keep, int32_t n_arrays, const float* const* src, float* const* dst,
+                          const int32_t* row_floats, void* workspace, size_t workspace_bytes, uint64_t* N_out_host,
+                          void* stream) {
+  MG_REQUIRE(N >= 0 && N < (int64_t)1 << 31, "N must be in [0, 2^31)");
+  MG_REQUIRE(n_arrays >= 0 && n_arrays <= 16, "n_arrays must be in 0..16");
+  MG_REQUIRE(workspace != nullptr && ((uintptr_t)workspace & 255) == 0, "workspace must be non-null and 256-byte aligned");
+  if (workspace_bytes < mg_compact_workspace_bytes(N)) {
+    mg_set_error("workspace too small: %zu bytes given, %zu needed", workspace_bytes, mg_compact_workspace_bytes(N));
+    return MG_ERR_CAPACITY;
+  }
+  cudaStream_t st = (cudaStream_t)stream;
+  char* ws = (char*)workspace;
+  unsigned long long* total = (unsigned long long*)ws;
+  const int nblk = (int)((N + CP_BLOCK - 1) / CP_BLOCK);
+  uint32_t* block_counts = (uint32_t*)(ws + align256(8));
+  uint32_t* pos = (uint32_t*)(ws + align256(8) + align256(4 * ((size_t)nblk + 1)));
+  MG_CHECK_CUDA(cudaMemsetAsync(total, 0, 8, st));
+  if (N > 0) {
+    MG_REQUIRE(keep && (n_arrays == 0 || (src && dst && row_floats)), "null array");
+    compact_count_kernel<<<nblk, CP_BLOCK, 0, st>>>(N, keep, block_counts);
+    compact_scan_kernel<<<1, 1024, 0, st>>>(block_counts, nblk, total);
+    compact_pos_kernel<<<nblk, CP_BLOCK, 0, st>>>(N, keep, block_counts, pos);
+    for (int a = 0; a < n_arrays; a++) {
+      MG_REQUIRE(src[a] && dst[a] && row_floats[a] > 0, "null array or non-positive row size");
+      const bool vec = row_floats[a] % 4 == 0 && ((uintptr_t)src[a] & 15) == 0 && ((uintptr_t)dst[a] & 15) == 0;
+      const int64_t r = vec ? row_floats[a] / 4 : row_floats[a];
+      const int64_t ne = N * r;
+      MG_REQUIRE(ne < ((int64_t)1 << 32) - MH_THREADS, "array too large for one compaction call (N * row size >= 2^32 elements)");
+      const unsigned grid = (unsigned)((ne + MH_THREADS - 1) / MH_THREADS);
+      if (vec) compact_rows_kernel<float4><<<grid, MH_THREADS, 0, st>>>((uint32_t)ne, (uint32_t)r, pos, (const float4*)src[a], (float4*)dst[a]);
+      else compact_rows_kernel<float><<<grid, MH_THREADS, 0, st>>>((uint32_t)ne, (uint32_t)r, pos, src[a], dst[a]);
+    }
+    MG_CHECK_LAUNCH();
+  }
+  if (N_out_host) MG_CHECK_CUDA(cudaMemcpyAsync(N_out_host, total, sizeof(uint64_t), cudaMemcpyDeviceToHost, st));
+  return MG_OK;
+}

@@ -146,7 +146,7 @@ __global__ void __launch_bounds__(PP_THREADS) preprocess_kernel(
   // 128-bit loads (a warp's 32 rows are contiguous), staged in shared memory, one row per lane
   const uint32_t vmask = __ballot_sync(0xffffffffu, touched > 0);
   if (nrows > 0 && vmask) {
-    if (L::VEC) {
+    if constexpr (L::VEC) {
       const float4* src = reinterpret_cast<const float4*>(sh + g0 * RK);
 #pragma unroll
       for (int k = 0; k < RK / 4; k++) {
@@ -166,7 +166,7 @@ __global__ void __launch_bounds__(PP_THREADS) preprocess_kernel(
   if (touched > 0) {
     const float* myrow = wrow + lane * STRIDE;
     float shv[RK];
-    if (L::VEC) {
+    if constexpr (L::VEC) {
 #pragma unroll
       for (int j = 0; j < RK / 4; j++) {
         const float4 v = *reinterpret_cast<const float4*>(myrow + 4 * j);

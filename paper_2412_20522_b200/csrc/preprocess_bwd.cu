@@ -118,7 +118,7 @@ __global__ void __launch_bounds__(PB_THREADS) preprocess_bwd_sh_kernel(
   }
   // coalesced load of the visible rows
   if (nrows > 0) {
-    if (L::VEC) {
+    if constexpr (L::VEC) {
       const float4* src = reinterpret_cast<const float4*>(sh + g0 * RK);
 #pragma unroll
       for (int k = 0; k < RK / 4; k++) {
@@ -150,7 +150,7 @@ __global__ void __launch_bounds__(PB_THREADS) preprocess_bwd_sh_kernel(
     float sj[K], Y[K];
     {
       float rowv[RK];
-      if (L::VEC) {
+      if constexpr (L::VEC) {
 #pragma unroll
         for (int j = 0; j < RK / 4; j++) {
           const float4 v = *reinterpret_cast<const float4*>(myrow + 4 * j);
@@ -204,7 +204,7 @@ __global__ void __launch_bounds__(PB_THREADS) preprocess_bwd_sh_kernel(
     for (int j = 0; j < K; j++) {
       out[3 * j] = Y[j] * gcol[0]; out[3 * j + 1] = Y[j] * gcol[1]; out[3 * j + 2] = Y[j] * gcol[2];
     }
-    if (L::VEC) {
+    if constexpr (L::VEC) {
 #pragma unroll
       for (int j = 0; j < RK / 4; j++)
         *reinterpret_cast<float4*>(myrow + 4 * j) = make_float4(out[4 * j], out[4 * j + 1], out[4 * j + 2], out[4 * j + 3]);
@@ -221,7 +221,7 @@ __global__ void __launch_bounds__(PB_THREADS) preprocess_bwd_sh_kernel(
   __syncwarp();
   // coalesced store of dL/dsh: rows of visible Gaussians from shared memory, zeros for the others
   if (nrows > 0) {
-    if (L::VEC) {
+    if constexpr (L::VEC) {
       float4* dst = reinterpret_cast<float4*>(dL_dsh + g0 * RK);
 #pragma unroll
       for (int k = 0; k < RK / 4; k++) {
