@@ -240,6 +240,40 @@ def bench_inference(sc, g, m, reps=30):
     return out
 
 
+def bench_cameras(sc, g, m, steps=10):
+    """BASELINE.json configs[4]: "Forward+backward are timed over 20 cameras on a circle".  ms per frame (all five
+    calls) for every camera of the scene; buffers sized for the largest R."""
+    import torch
+
+    from paper_2412_20522_b200 import binding as mg
+
+    fr = mg.Frame(sc.cameras[0], sc.N)
+    Rs = []
+    for cam in sc.cameras:
+        fr.set_camera(cam)
+        fr.preprocess(g)
+        torch.cuda.current_stream().synchronize()
+        Rs.append(int(fr.R_host[0]))
+    fr.reserve(max(Rs))
+    ms = []
+    for ci, cam in enumerate(sc.cameras):
+        fr.set_camera(cam)
+        gimg = torch.from_numpy(sc.dL_dimage(ci)).cuda()
+        for _ in range(2):
+            fr.step(g, m, gimg)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(steps):
+            fr.step(g, m, gimg)
+        e1.record()
+        torch.cuda.synchronize()
+        ms.append(e0.elapsed_time(e1) / steps)
+        assert int(fr.R_host[1]) == Rs[ci]
+    return {"cameras": len(ms), "ms_per_frame_mean": float(np.mean(ms)), "ms_per_frame_max": float(np.max(ms)),
+            "ms_per_frame_min": float(np.min(ms)), "R_min": min(Rs), "R_max": max(Rs)}
+
+
 def n_threads():
     try:
         return len(os.sched_getaffinity(0))
@@ -288,6 +322,7 @@ def main():
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--all-cameras", action="store_true", help="also time every camera of the scene (config 5: 20)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", 0))
     world = int(os.environ.get("WORLD_SIZE", 1))
@@ -468,6 +503,9 @@ def main():
     if os.path.exists(peaks_path):
         hbm_gbs = float(json.load(open(peaks_path)).get("hbm_gbs", hbm_gbs))
     next_rows = {"mask_head": bench_mask_head(sc, g, hbm_gbs), "inference": bench_inference(sc, g, m)} if world == 1 else None
+
+    if args.all_cameras and world == 1 and next_rows is not None:
+        next_rows["all_cameras"] = bench_cameras(sc, g, m)
 
     cpu = None
     if not args.no_cpu_baseline:

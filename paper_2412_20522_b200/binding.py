@@ -222,6 +222,13 @@ class Frame:
         self.sorted_ids = None
         self.workspace = None
 
+    def set_camera(self, cam_like):
+        """Point the frame at another camera of the same image size (buffers are reused)."""
+        assert (cam_like.width, cam_like.height, cam_like.sh_degree) == (self.cam_like.width, self.cam_like.height,
+                                                                         self.cam_like.sh_degree)
+        self.cam_like = cam_like
+        self.cam = camera(cam_like)
+
     def reserve(self, R_capacity):
         """(Re)allocate sorted_ids and the sort workspace for at most R_capacity duplicated keys."""
         if R_capacity > self.R_capacity or self.sorted_ids is None:
