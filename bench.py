@@ -274,6 +274,37 @@ def bench_cameras(sc, g, m, steps=10):
             "ms_per_frame_min": float(np.min(ms)), "R_min": min(Rs), "R_max": max(Rs)}
 
 
+def bench_render_loss(sc, hbm_gbs, reps=30):
+    """SURVEY.md 8(f) row f3 at the bench image size.  Algorithmic bytes per image element: 12 (image and target in,
+    gradient out); the two-kernel scheme moves 44 (three derivative maps written and read back)."""
+    import torch
+
+    from paper_2412_20522_b200 import binding as mg
+
+    cam = sc.camera
+    rng = np.random.default_rng(3)
+    img = torch.from_numpy(rng.uniform(0, 1, (3, cam.height, cam.width)).astype(np.float32)).cuda()
+    tgt = torch.from_numpy(rng.uniform(0, 1, (3, cam.height, cam.width)).astype(np.float32)).cuda()
+    grad = torch.empty_like(img)
+    stats = torch.zeros(3, dtype=torch.float64, device="cuda")
+    ws = torch.empty(mg.mg_render_loss_workspace_bytes(cam.width, cam.height), dtype=torch.uint8, device="cuda")
+    fn = lambda: mg.mg_render_loss(img, tgt, 0.2, grad, stats, ws)
+    for _ in range(3):
+        fn()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(reps):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / reps
+    n = img.numel()
+    return {"image": [cam.width, cam.height], "ms": round(ms, 4), "algorithmic_gb_per_s": round(12 * n / (ms * 1e-3) / 1e9, 1),
+            "moved_gb_per_s": round(44 * n / (ms * 1e-3) / 1e9, 1), "frac_of_hbm_peak": round(12 * n / (ms * 1e-3) / 1e9 / hbm_gbs, 4),
+            "note": "13 MB per plane set: L2-resident, launch- and latency-bound at this size"}
+
+
 def n_threads():
     try:
         return len(os.sched_getaffinity(0))
@@ -502,7 +533,8 @@ def main():
     hbm_gbs = 6540.8
     if os.path.exists(peaks_path):
         hbm_gbs = float(json.load(open(peaks_path)).get("hbm_gbs", hbm_gbs))
-    next_rows = {"mask_head": bench_mask_head(sc, g, hbm_gbs), "inference": bench_inference(sc, g, m)} if world == 1 else None
+    next_rows = {"mask_head": bench_mask_head(sc, g, hbm_gbs), "inference": bench_inference(sc, g, m),
+                 "render_loss": bench_render_loss(sc, hbm_gbs)} if world == 1 else None
 
     if args.all_cameras and world == 1 and next_rows is not None:
         next_rows["all_cameras"] = bench_cameras(sc, g, m)

@@ -169,6 +169,17 @@ size_t mg_compact_workspace_bytes(int64_t N);
 int mg_compact(int64_t N, const uint8_t* keep, int32_t n_arrays, const float* const* src, float* const* dst,
                const int32_t* row_floats, void* workspace, size_t workspace_bytes, uint64_t* N_out_host, void* stream);
 
+/* ---- The render loss.  Eq. 8: L = L_render + lambda_m L_m with L_render
+ * "the original rendering loss", which the paper does not define; reading 26: the loss of the 3DGS method the paper
+ * modifies, L_render = (1 - lambda) mean|I - G| + lambda (1 - mean SSIM(I, G)), SSIM per channel with a
+ * separable 11-tap Gaussian window (sigma 1.5, normalised), zero padding, C1 = 0.01^2, C2 = 0.03^2, means over all
+ * 3 H W elements.  image, target, dL_dimage: planar [3][H][W]; dL_dimage = dL_render/dimage is overwritten.
+ * stats (DEVICE, 3 doubles, overwritten): mean|I - G|, mean SSIM, L_render.
+ * workspace: mg_render_loss_workspace_bytes(width, height) bytes of device memory. */
+size_t mg_render_loss_workspace_bytes(int32_t width, int32_t height);
+int mg_render_loss(int32_t width, int32_t height, const float* image, const float* target, float lambda_dssim,
+                   float* dL_dimage, double* stats, void* workspace, size_t workspace_bytes, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -34,7 +34,8 @@ class mg_camera(C.Structure):
 
 EXPORTS = ["mg_last_error_string", "mg_version", "mg_workspace_bytes", "mg_preprocess", "mg_bin_sort",
            "mg_render_fwd", "mg_render_bwd", "mg_preprocess_bwd", "mg_mask_sample", "mg_mask_sample_bwd", "mg_mask_loss",
-           "mg_mask_prune_keep", "mg_compact_workspace_bytes", "mg_compact"]
+           "mg_mask_prune_keep", "mg_compact_workspace_bytes", "mg_compact", "mg_render_loss_workspace_bytes",
+           "mg_render_loss"]
 
 
 def lib():
@@ -48,10 +49,12 @@ def lib():
         L.mg_last_error_string.restype = C.c_char_p
         L.mg_workspace_bytes.restype = C.c_size_t
         L.mg_workspace_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int32, C.c_uint64]
+        L.mg_render_loss_workspace_bytes.restype = C.c_size_t
+        L.mg_render_loss_workspace_bytes.argtypes = [C.c_int32, C.c_int32]
         L.mg_compact_workspace_bytes.restype = C.c_size_t
         L.mg_compact_workspace_bytes.argtypes = [C.c_int64]
         for name in EXPORTS[3:]:
-            if name != "mg_compact_workspace_bytes":
+            if not name.endswith("_workspace_bytes"):
                 getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
@@ -189,6 +192,17 @@ def mg_compact(keep, src, dst, workspace, N_out_host=None):
         assert t.is_contiguous() and t.dtype == F32 and t.device.type == "cuda"
     _check(lib().mg_compact(C.c_int64(N), _ptr(keep, U8), C.c_int32(n), srcp, dstp, rows, _ptr(workspace, U8),
                             C.c_size_t(workspace.numel()), _ptr(N_out_host, torch.int64, "cpu"), _stream()))
+
+
+def mg_render_loss_workspace_bytes(width, height) -> int:
+    return int(lib().mg_render_loss_workspace_bytes(int(width), int(height)))
+
+
+def mg_render_loss(image, target, lambda_dssim, dL_dimage, stats, workspace):
+    _, H, W = image.shape
+    _check(lib().mg_render_loss(C.c_int32(W), C.c_int32(H), _ptr(image, F32), _ptr(target, F32), C.c_float(lambda_dssim),
+                                _ptr(dL_dimage, F32), _ptr(stats, torch.float64), _ptr(workspace, U8),
+                                C.c_size_t(workspace.numel()), _stream()))
 
 
 class Frame:
