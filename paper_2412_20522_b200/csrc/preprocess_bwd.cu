@@ -106,16 +106,18 @@ __global__ void __launch_bounds__(PB_THREADS) preprocess_bwd_sh_kernel(
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const int64_t g0 = i - lane;                              // first Gaussian of this warp
   const int nrows = (int)max((int64_t)0, min((int64_t)32, N - g0));
-  const bool vis = i < N && radii[i] > 0;
-  const uint32_t vmask = __ballot_sync(0xffffffffu, vis);
-  // this thread's own small inputs first, so that they are in flight together with the rows
+  // A Gaussian whose colour received no gradient (culled, every channel clamped, or -- the common case -- never
+  // reached by a pixel before the pixel saturated) has dL/dsh = 0 and no direction term: its row is not read.
+  bool vis = i < N && radii[i] > 0;
   float px = 0.f, py = 0.f, pz = 0.f, gcol[3] = {0.f, 0.f, 0.f};
   if (vis) {
-    px = means[3 * i]; py = means[3 * i + 1]; pz = means[3 * i + 2];
     const uint32_t cl = clamped[i];
 #pragma unroll
     for (int k = 0; k < 3; k++) gcol[k] = (cl >> k & 1u) ? 0.f : dL_drgb[3 * i + k];
+    vis = gcol[0] != 0.f || gcol[1] != 0.f || gcol[2] != 0.f;
+    if (vis) { px = means[3 * i]; py = means[3 * i + 1]; pz = means[3 * i + 2]; }
   }
+  const uint32_t vmask = __ballot_sync(0xffffffffu, vis);
   // coalesced load of the visible rows
   if (nrows > 0) {
     if constexpr (L::VEC) {
@@ -259,12 +261,20 @@ __global__ void __launch_bounds__(PB_THREADS, PB_MINB) preprocess_bwd_geo_kernel
     dL_dopacity_logits[i] = 0.f;
     return;
   }
+  const float2 gm = dL_dmeans2d[i];
+  const float gA = dL_dconic[3 * i], gB = dL_dconic[3 * i + 1], gC = dL_dconic[3 * i + 2];
+  const float go = dL_dopacity[i];
+  if (gm.x == 0.f && gm.y == 0.f && gA == 0.f && gB == 0.f && gC == 0.f && go == 0.f) {
+    // no gradient reached this Gaussian (no pixel blended it before saturating): every product below is zero
+    dL_dlog_scales[3 * i] = dL_dlog_scales[3 * i + 1] = dL_dlog_scales[3 * i + 2] = 0.f;
+    dL_dquats[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    dL_dopacity_logits[i] = 0.f;
+    return;
+  }
   const float px = means[3 * i], py = means[3 * i + 1], pz = means[3 * i + 2];
   const float4 q = __ldg(reinterpret_cast<const float4*>(quats) + i);
   const double s0 = exp((double)log_scales[3 * i]), s1 = exp((double)log_scales[3 * i + 1]), s2 = exp((double)log_scales[3 * i + 2]);
   const float o = 1.f / (1.f + expf(-opacity_logits[i]));
-  const float2 gm = dL_dmeans2d[i];
-  const float gA = dL_dconic[3 * i], gB = dL_dconic[3 * i + 1], gC = dL_dconic[3 * i + 2];
   const float dmx = dL_dmeans[3 * i], dmy = dL_dmeans[3 * i + 1], dmz = dL_dmeans[3 * i + 2];  // colour part
 
   // ---------------- geometry: forward chain and dL/dconic -> dL/dU in fp64 ----------------
@@ -329,7 +339,7 @@ __global__ void __launch_bounds__(PB_THREADS, PB_MINB) preprocess_bwd_geo_kernel
   dL_dlog_scales[3 * i] = gg.dls[0]; dL_dlog_scales[3 * i + 1] = gg.dls[1]; dL_dlog_scales[3 * i + 2] = gg.dls[2];
   dL_dquats[i] = gg.dq;
   dL_dmeans[3 * i] = gg.dm[0]; dL_dmeans[3 * i + 1] = gg.dm[1]; dL_dmeans[3 * i + 2] = gg.dm[2];
-  dL_dopacity_logits[i] = dL_dopacity[i] * o * ((G)1. - o);
+  dL_dopacity_logits[i] = go * o * ((G)1. - o);
 }
 
 }  // namespace
