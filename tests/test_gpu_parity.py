@@ -264,3 +264,52 @@ def test_tile_order_does_not_change_the_image(run):
                      fr.final_T, fr.n_contrib, tile_order=None)
     torch.cuda.synchronize()
     assert torch.equal(img, fr.image) and torch.equal(fT, fr.final_T) and torch.equal(nc, fr.n_contrib)
+
+
+@pytest.mark.parametrize("seed,W,H,n,big_frac,tie_levels", [
+    (0, 16, 16, 500, 0.5, 3),          # a single tile, heavy depth ties
+    (1, 530, 40, 3000, 0.1, 0),        # 34 x 3 tiles: two 32-bin words in x, one in y
+    (2, 40, 1100, 3000, 0.1, 50),      # 3 x 69 tiles: three words in y
+    (3, 2100, 2100, 40_000, 0.02, 0),  # 132 x 132 tiles: five words both ways
+    (4, 1297, 840, 200_000, 0.05, 1000),
+    (5, 333, 211, 70_000, 1.0, 7),     # every rect is large: long runs per record
+])
+def test_bin_sort_random_rects_through_the_c_abi(oracle, seed, W, H, n, big_frac, tie_levels):
+    """mg_bin_sort alone on synthetic (depth, rect) inputs that the projection would not produce together: depth
+    ties (order by index), rects of every shape incl. whole-image ones, culled entries, odd grid shapes -- compared
+    bit for bit with the oracle's list builder."""
+    rng = np.random.default_rng(seed)
+    cam0 = scenes.config1().camera
+    cam = scenes.Camera(W, H, 100.0, 100.0, W / 2, H / 2, cam0.R, cam0.t, sh_degree=0)
+    gw, gh = mg.grid(cam)
+    x0 = rng.integers(0, gw, n)
+    y0 = rng.integers(0, gh, n)
+    big = rng.uniform(size=n) < big_frac
+    wx = np.where(big, rng.integers(1, gw + 1, n), rng.integers(1, 4, n))
+    wy = np.where(big, rng.integers(1, gh + 1, n), rng.integers(1, 4, n))
+    x1, y1 = np.minimum(x0 + wx, gw), np.minimum(y0 + wy, gh)
+    culled = rng.uniform(size=n) < 0.2
+    rects = np.stack([x0, y0, x1, y1], 1).astype(np.int32)
+    rects[culled] = 0
+    tt = ((rects[:, 2] - rects[:, 0]) * (rects[:, 3] - rects[:, 1])).astype(np.uint32)
+    depths = rng.uniform(0.3, 50.0, n).astype(np.float32)
+    if tie_levels:
+        depths = (np.round(depths * tie_levels / 50.0) * (50.0 / tie_levels) + 0.25).astype(np.float32)
+    R = int(tt.astype(np.int64).sum())
+    ids_ref, ranges_ref = orc_bin_sort(oracle, cam, depths, rects, tt)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    ws = torch.empty(mg.mg_workspace_bytes(n, W, H, R), dtype=torch.uint8, device="cuda")
+    sorted_ids = torch.empty(max(R, 1), dtype=torch.int32, device="cuda")
+    ranges = torch.empty(gw * gh, 2, dtype=torch.int32, device="cuda")
+    order = torch.empty(gw * gh, dtype=torch.int32, device="cuda")
+    R_host = torch.zeros(1, dtype=torch.int64).pin_memory()
+    mg.mg_bin_sort(mg.camera(cam), d(depths), d(rects), d(tt.view(np.int32)), R, ws, sorted_ids, ranges, R_host, order)
+    torch.cuda.synchronize()
+    assert int(R_host[0]) == R
+    assert np.array_equal(pu.u32(ranges), ranges_ref)
+    assert np.array_equal(pu.u32(sorted_ids)[:R], ids_ref)
+    assert sorted(order.cpu().numpy().tolist()) == list(range(gw * gh))
+
+
+def orc_bin_sort(oracle, cam, depths, rects, tt):
+    return oracle.bin_sort(cam, depths, rects, tt)
