@@ -247,30 +247,16 @@ __global__ void __launch_bounds__(PB_THREADS) preprocess_bwd_sh_kernel(
 
 
 // Kernel 2 of 2: geometry.  Adds its part to dL_dmeans (written by kernel 1) and writes the other gradients.
-__global__ void __launch_bounds__(PB_THREADS, PB_MINB) preprocess_bwd_geo_kernel(
-    mg_camera cam, int64_t N, const float* __restrict__ means, const float* __restrict__ log_scales,
-    const float* __restrict__ quats, const float* __restrict__ opacity_logits, const int32_t* __restrict__ radii,
-    const float2* __restrict__ dL_dmeans2d, const float* __restrict__ dL_dconic, const float* __restrict__ dL_dopacity,
-    float* __restrict__ dL_dmeans, float* __restrict__ dL_dlog_scales, float4* __restrict__ dL_dquats,
-    float* __restrict__ dL_dopacity_logits) {
-  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= N) return;
-  if (radii[i] <= 0) {  // culled: exact zeros everywhere (dL_dmeans was zeroed by kernel 1)
-    dL_dlog_scales[3 * i] = dL_dlog_scales[3 * i + 1] = dL_dlog_scales[3 * i + 2] = 0.f;
-    dL_dquats[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-    dL_dopacity_logits[i] = 0.f;
-    return;
-  }
+// The chain of one Gaussian:
+__device__ __forceinline__ void geo_one(const mg_camera& cam, int64_t i, const float* __restrict__ means,
+                                        const float* __restrict__ log_scales, const float* __restrict__ quats,
+                                        const float* __restrict__ opacity_logits, const float2* __restrict__ dL_dmeans2d,
+                                        const float* __restrict__ dL_dconic, const float* __restrict__ dL_dopacity,
+                                        float* __restrict__ dL_dmeans, float* __restrict__ dL_dlog_scales,
+                                        float4* __restrict__ dL_dquats, float* __restrict__ dL_dopacity_logits) {
   const float2 gm = dL_dmeans2d[i];
   const float gA = dL_dconic[3 * i], gB = dL_dconic[3 * i + 1], gC = dL_dconic[3 * i + 2];
   const float go = dL_dopacity[i];
-  if (gm.x == 0.f && gm.y == 0.f && gA == 0.f && gB == 0.f && gC == 0.f && go == 0.f) {
-    // no gradient reached this Gaussian (no pixel blended it before saturating): every product below is zero
-    dL_dlog_scales[3 * i] = dL_dlog_scales[3 * i + 1] = dL_dlog_scales[3 * i + 2] = 0.f;
-    dL_dquats[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-    dL_dopacity_logits[i] = 0.f;
-    return;
-  }
   const float px = means[3 * i], py = means[3 * i + 1], pz = means[3 * i + 2];
   const float4 q = __ldg(reinterpret_cast<const float4*>(quats) + i);
   const double s0 = exp((double)log_scales[3 * i]), s1 = exp((double)log_scales[3 * i + 1]), s2 = exp((double)log_scales[3 * i + 2]);
@@ -342,6 +328,95 @@ __global__ void __launch_bounds__(PB_THREADS, PB_MINB) preprocess_bwd_geo_kernel
   dL_dopacity_logits[i] = go * o * ((G)1. - o);
 }
 
+// Only Gaussians that received a gradient need the chain, and once the pixels saturate few do (1 in 5 at config 3,
+// scattered over the array), so the kernel is a persistent grid whose blocks sweep a contiguous range: a sweep
+// step writes the zeros of 256 Gaussians that need none and appends the indices of the others to a queue in
+// shared memory; whenever the queue holds 256 indices, all 8 warps run the fp64 chain on full lanes.
+constexpr int PG_THREADS = 256;
+constexpr int PG_SWEEP = 4;  // Gaussians per thread and sweep step
+
+__global__ void __launch_bounds__(PG_THREADS, 2) preprocess_bwd_geo_kernel(
+    mg_camera cam, int64_t N, const float* __restrict__ means, const float* __restrict__ log_scales,
+    const float* __restrict__ quats, const float* __restrict__ opacity_logits, const int32_t* __restrict__ radii,
+    const float2* __restrict__ dL_dmeans2d, const float* __restrict__ dL_dconic, const float* __restrict__ dL_dopacity,
+    float* __restrict__ dL_dmeans, float* __restrict__ dL_dlog_scales, float4* __restrict__ dL_dquats,
+    float* __restrict__ dL_dopacity_logits) {
+  __shared__ uint32_t queue[(PG_SWEEP + 1) * PG_THREADS];  // indices relative to the block's range
+  __shared__ uint32_t wcount[PG_THREADS / 32];
+  __shared__ uint32_t qn;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  constexpr int STEP = PG_SWEEP * PG_THREADS;
+  const int64_t per = ((N + gridDim.x - 1) / gridDim.x + STEP - 1) / STEP * STEP;
+  const int64_t begin = (int64_t)blockIdx.x * per, end = min(N, begin + per);
+  if (threadIdx.x == 0) qn = 0;
+  __syncthreads();
+  int64_t i0 = begin;
+  for (;;) {
+    if (i0 < end) {
+      // sweep PG_SWEEP x 256 Gaussians: all their loads are in flight together
+      // every load is issued before any is tested (no short-circuit: dependent loads would serialise the latency)
+      bool active[PG_SWEEP];
+      int rad[PG_SWEEP];
+      float2 gm_[PG_SWEEP];
+      float gc_[PG_SWEEP][3], go_[PG_SWEEP];
+#pragma unroll
+      for (int u = 0; u < PG_SWEEP; u++) {
+        const int64_t i = i0 + u * PG_THREADS + threadIdx.x;
+        const bool in = i < end;
+        rad[u] = in ? radii[i] : 0;
+        gm_[u] = in ? dL_dmeans2d[i] : make_float2(0.f, 0.f);
+        gc_[u][0] = in ? dL_dconic[3 * i] : 0.f;
+        gc_[u][1] = in ? dL_dconic[3 * i + 1] : 0.f;
+        gc_[u][2] = in ? dL_dconic[3 * i + 2] : 0.f;
+        go_[u] = in ? dL_dopacity[i] : 0.f;
+      }
+#pragma unroll
+      for (int u = 0; u < PG_SWEEP; u++)
+        active[u] = rad[u] > 0 && ((gm_[u].x != 0.f) | (gm_[u].y != 0.f) | (gc_[u][0] != 0.f) | (gc_[u][1] != 0.f) |
+                                   (gc_[u][2] != 0.f) | (go_[u] != 0.f));
+#pragma unroll
+      for (int u = 0; u < PG_SWEEP; u++) {
+        const int64_t i = i0 + u * PG_THREADS + threadIdx.x;
+        if (i < end && !active[u]) {
+          // culled, or no gradient reached this Gaussian (no pixel blended it before saturating): exact zeros
+          // (dL_dmeans holds the colour part, zero as well, from kernel 1)
+          dL_dlog_scales[3 * i] = dL_dlog_scales[3 * i + 1] = dL_dlog_scales[3 * i + 2] = 0.f;
+          dL_dquats[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+          dL_dopacity_logits[i] = 0.f;
+        }
+        const uint32_t ballot = __ballot_sync(0xffffffffu, active[u]);
+        if (lane == 0) wcount[warp] = __popc(ballot);
+        __syncthreads();
+        uint32_t off = qn, tot = 0;
+#pragma unroll
+        for (int w = 0; w < PG_THREADS / 32; w++) {
+          if (w < warp) off += wcount[w];
+          tot += wcount[w];
+        }
+        if (active[u]) queue[off + __popc(ballot & ((1u << lane) - 1u))] = (uint32_t)(i - begin);
+        __syncthreads();
+        if (threadIdx.x == 0) qn += tot;
+        __syncthreads();
+      }
+      i0 += STEP;
+    }
+    const uint32_t n = qn;  // same value in every thread
+    const bool flush = i0 >= end;
+    if (n >= PG_THREADS || (flush && n > 0)) {
+      // run the chain on the LAST min(n, 256) entries of the queue: nothing to move afterwards
+      const uint32_t cnt = min(n, (uint32_t)PG_THREADS);
+      if (threadIdx.x < cnt)
+        geo_one(cam, begin + queue[n - cnt + threadIdx.x], means, log_scales, quats, opacity_logits, dL_dmeans2d, dL_dconic,
+                dL_dopacity, dL_dmeans, dL_dlog_scales, dL_dquats, dL_dopacity_logits);
+      __syncthreads();
+      if (threadIdx.x == 0) qn = n - cnt;
+      __syncthreads();
+    } else if (flush) {
+      break;
+    }
+  }
+}
+
 }  // namespace
 
 extern "C" int mg_preprocess_bwd(const mg_camera* cam, int64_t N, const float* means, const float* log_scales,
@@ -369,7 +444,15 @@ extern "C" int mg_preprocess_bwd(const mg_camera* cam, int64_t N, const float* m
   }
 #undef MG_LAUNCH
   MG_CHECK_LAUNCH();
-  preprocess_bwd_geo_kernel<<<blocks, threads, 0, st>>>(*cam, N, means, log_scales, quats, opacity_logits, radii,
+  static int geo_grid = 0;
+  if (geo_grid == 0) {
+    int dev = 0, sms = 0;
+    MG_CHECK_CUDA(cudaGetDevice(&dev));
+    MG_CHECK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    geo_grid = 2 * sms;
+  }
+  const int64_t geo_want = (N + PG_THREADS - 1) / PG_THREADS;
+  preprocess_bwd_geo_kernel<<<(unsigned)(geo_want < geo_grid ? geo_want : geo_grid), PG_THREADS, 0, st>>>(*cam, N, means, log_scales, quats, opacity_logits, radii,
                                                         (const float2*)dL_dmeans2d, dL_dconic, dL_dopacity, dL_dmeans,
                                                         dL_dlog_scales, (float4*)dL_dquats, dL_dopacity_logits);
   MG_CHECK_LAUNCH();
