@@ -108,15 +108,18 @@ __global__ void __launch_bounds__(PB_THREADS) preprocess_bwd_sh_kernel(
   const int nrows = (int)max((int64_t)0, min((int64_t)32, N - g0));
   // A Gaussian whose colour received no gradient (culled, every channel clamped, or -- the common case -- never
   // reached by a pixel before the pixel saturated) has dL/dsh = 0 and no direction term: its row is not read.
-  bool vis = i < N && radii[i] > 0;
-  float px = 0.f, py = 0.f, pz = 0.f, gcol[3] = {0.f, 0.f, 0.f};
-  if (vis) {
-    const uint32_t cl = clamped[i];
+  // (every small load is issued before any is tested: dependent loads would serialise their latencies)
+  const bool in = i < N;
+  const int rad = in ? radii[i] : 0;
+  const uint32_t cl = in ? clamped[i] : 7u;
+  float gcol[3];
 #pragma unroll
-    for (int k = 0; k < 3; k++) gcol[k] = (cl >> k & 1u) ? 0.f : dL_drgb[3 * i + k];
-    vis = gcol[0] != 0.f || gcol[1] != 0.f || gcol[2] != 0.f;
-    if (vis) { px = means[3 * i]; py = means[3 * i + 1]; pz = means[3 * i + 2]; }
-  }
+  for (int k = 0; k < 3; k++) gcol[k] = in ? dL_drgb[3 * i + k] : 0.f;
+  const float px = in ? means[3 * i] : 0.f, py = in ? means[3 * i + 1] : 0.f, pz = in ? means[3 * i + 2] : 0.f;
+#pragma unroll
+  for (int k = 0; k < 3; k++)
+    if (cl >> k & 1u) gcol[k] = 0.f;
+  const bool vis = rad > 0 && ((gcol[0] != 0.f) | (gcol[1] != 0.f) | (gcol[2] != 0.f));
   const uint32_t vmask = __ballot_sync(0xffffffffu, vis);
   // coalesced load of the visible rows
   if (nrows > 0) {
