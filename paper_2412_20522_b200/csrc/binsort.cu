@@ -48,6 +48,7 @@ constexpr int RS_BINS = 256;
 #define XP_CHUNK_ 128
 #endif
 constexpr int XP_CHUNK = XP_CHUNK_;   // items per warp in the expansion sweeps
+constexpr int XP_GROUPS = XP_CHUNK / 32;
 constexpr int XP_MAX_WARPS = 8; // warps per block in the expansion sweeps
 constexpr int SCAN_THREADS = 1024;
 constexpr int SCAN_ITEMS = 4;
@@ -476,26 +477,39 @@ __global__ void __launch_bounds__(32 * XP_MAX_WARPS) row_expand_kernel(
   __syncwarp();
   if (k0 < nvis) {
     const uint32_t k1 = min(k0 + (uint32_t)XP_CHUNK, nvis);
-    for (uint32_t kb = k0; kb < k1; kb += 32) {
-      const uint32_t k = kb + lane;
-      uint32_t id = 0, xx = 0;
-      int lo = 0, hi = 0;
+    // all loads of the chunk are issued before the first group is processed (XP_GROUPS items per lane)
+    uint32_t id[XP_GROUPS], xx[XP_GROUPS], yy[XP_GROUPS];
+#pragma unroll
+    for (int u = 0; u < XP_GROUPS; u++) {
+      const uint32_t k = k0 + 32 * u + lane;
+      id[u] = k < k1 ? order[k] : 0u;
+    }
+#pragma unroll
+    for (int u = 0; u < XP_GROUPS; u++) {
+      const uint32_t k = k0 + 32 * u + lane;
+      xx[u] = 0; yy[u] = 0;
       if (k < k1) {
         if (kCount) {
-          id = order[k];
-          const int4 r = rects[id];
-          xx = (uint32_t)r.x | ((uint32_t)r.z << 16);
-          lo = r.y; hi = r.w;
-          prect[k] = make_uint2(xx, (uint32_t)r.y | ((uint32_t)r.w << 16));
+          const int4 r = rects[id[u]];
+          xx[u] = (uint32_t)r.x | ((uint32_t)r.z << 16);
+          yy[u] = (uint32_t)r.y | ((uint32_t)r.w << 16);
         } else {
-          id = order[k];
           const uint2 p = prect[k];
-          xx = p.x;
-          lo = (int)(p.y & 0xffffu); hi = (int)(p.y >> 16);
+          xx[u] = p.x; yy[u] = p.y;
         }
       }
-      if (kCount) xp_count_group(lo, hi, cnt);
-      else xp_emit_group<2>(lo, hi, id, xx, cnt, lane, reinterpret_cast<uint32_t*>(row_rec));
+    }
+#pragma unroll
+    for (int u = 0; u < XP_GROUPS; u++) {
+      const uint32_t k = k0 + 32 * u + lane;
+      if (k0 + 32 * u >= k1) break;
+      const int lo = (int)(yy[u] & 0xffffu), hi = (int)(yy[u] >> 16);  // empty interval for lanes past the end
+      if (kCount) {
+        if (k < k1) prect[k] = make_uint2(xx[u], yy[u]);
+        xp_count_group(lo, hi, cnt);
+      } else {
+        xp_emit_group<2>(lo, hi, id[u], xx[u], cnt, lane, reinterpret_cast<uint32_t*>(row_rec));
+      }
     }
   }
   if (kCount) {
@@ -567,17 +581,18 @@ __global__ void __launch_bounds__(32 * XP_MAX_WARPS) col_expand_kernel(
   uint32_t* tab = table_c + (size_t)gw * cb + c;
   for (int b = lane; b <= gw; b += 32) cnt[b] = (kCount || b == gw) ? 0u : tab[(size_t)b * nch];
   __syncwarp();
-  for (uint32_t jb = j0; jb < j1; jb += 32) {
-    const uint32_t j = jb + lane;
-    uint32_t id = 0;
-    int lo = 0, hi = 0;
-    if (j < j1) {
-      const uint2 rec = row_rec[j];
-      id = rec.x;
-      lo = (int)(rec.y & 0xffffu); hi = (int)(rec.y >> 16);
-    }
+  uint2 rec[XP_GROUPS];  // all records of the chunk are loaded before the first group is processed
+#pragma unroll
+  for (int u = 0; u < XP_GROUPS; u++) {
+    const uint32_t j = j0 + 32 * u + lane;
+    rec[u] = j < j1 ? row_rec[j] : make_uint2(0u, 0u);
+  }
+#pragma unroll
+  for (int u = 0; u < XP_GROUPS; u++) {
+    if (j0 + 32 * u >= j1) break;
+    const int lo = (int)(rec[u].y & 0xffffu), hi = (int)(rec[u].y >> 16);
     if (kCount) xp_count_group(lo, hi, cnt);
-    else xp_emit_group<1>(lo, hi, id, 0u, cnt, lane, sorted_ids);
+    else xp_emit_group<1>(lo, hi, rec[u].x, 0u, cnt, lane, sorted_ids);
   }
   if (kCount) {
     __syncwarp();
