@@ -184,13 +184,13 @@ __global__ void __launch_bounds__(RN_THREADS, RN_BWD_MINB) render_bwd_kernel(
 #pragma unroll
         for (int k = 0; k < 4; k++) {
           if ((sb >> k) & 1u) {
+            // branch-free: a pair that fails the filter gets alpha = 0 and adds nothing
             const float e = rn_eval(p, ra.w, k);
-            if (rn_filter(e, lo) && pos <= last[k]) {
-              const float alpha = fminf(MG_ALPHA_MAX, rn_ex2(e));
-              const float gc = g0[k] * rc.x + g1[k] * rc.y + g2[k] * rc.z;
-              const float X = kBg ? T[k] * (gc - gB[k]) - tfg[k] : T[k] * (gc - gB[k]);
-              dm = fmaf(alpha, X, dm);
-            }
+            const bool pass = rn_filter(e, lo) && pos <= last[k];
+            const float alpha = pass ? fminf(MG_ALPHA_MAX, rn_ex2(e)) : 0.f;
+            const float gc = g0[k] * rc.x + g1[k] * rc.y + g2[k] * rc.z;
+            const float X = kBg ? T[k] * (gc - gB[k]) - tfg[k] : T[k] * (gc - gB[k]);
+            dm = fmaf(alpha, X, dm);
           }
         }
         if (__any_sync(0xffffffffu, dm != 0.f)) {
@@ -210,32 +210,30 @@ __global__ void __launch_bounds__(RN_THREADS, RN_BWD_MINB) render_bwd_kernel(
           const bool pass = rn_filter(e, lo) && pos <= last[k];
           if (__any_sync(0xffffffffu, pass)) {
             contrib = true;
-            if (pass) {
-              const float raw_alpha = rn_ex2(e);
-              const float alpha = fminf(MG_ALPHA_MAX, raw_alpha);
-              const float a = m * alpha;
-              const float oma = 1.f - a;
-              const float inv = rn_rcp(oma);
-              const float Ti = T[k] * inv;
-              const float gc = g0[k] * rc.x + g1[k] * rc.y + g2[k] * rc.z;
-              const float X = kBg ? Ti * (gc - gB[k]) - tfg[k] * inv : Ti * (gc - gB[k]);
-              dm = fmaf(alpha, X, dm);
-              const float wgt = a * Ti;
-              dr = fmaf(wgt, g0[k], dr);
-              dg = fmaf(wgt, g1[k], dg);
-              db = fmaf(wgt, g2[k], db);
-              gB[k] = fmaf(a, gc, oma * gB[k]);
-              T[k] = Ti;
-              if (raw_alpha <= MG_ALPHA_MAX) {
-                const float q = alpha * (m * X);
-                const float ddx = p.dx[k & 1], ddy = p.dy[k >> 1];
-                const float qx = q * ddx, qy = q * ddy;
-                S += q; Sx += qx; Sy += qy;
-                Sxx = fmaf(qx, ddx, Sxx);
-                Sxy = fmaf(qx, ddy, Sxy);
-                Syy = fmaf(qy, ddy, Syy);
-              }
-            }
+            // branch-free inside the section: a lane whose pair fails the filter blends with alpha = 0, which adds
+            // nothing to any sum; its T and g.b are kept by a select
+            const float raw_alpha = rn_ex2(e);
+            const float alpha = pass ? fminf(MG_ALPHA_MAX, raw_alpha) : 0.f;
+            const float a = m * alpha;
+            const float oma = 1.f - a;
+            const float inv = rn_rcp(oma);
+            const float Ti = T[k] * inv;
+            const float gc = g0[k] * rc.x + g1[k] * rc.y + g2[k] * rc.z;
+            const float X = kBg ? Ti * (gc - gB[k]) - tfg[k] * inv : Ti * (gc - gB[k]);
+            dm = fmaf(alpha, X, dm);
+            const float wgt = a * Ti;
+            dr = fmaf(wgt, g0[k], dr);
+            dg = fmaf(wgt, g1[k], dg);
+            db = fmaf(wgt, g2[k], db);
+            gB[k] = pass ? fmaf(a, gc, oma * gB[k]) : gB[k];
+            T[k] = pass ? Ti : T[k];
+            const float q = raw_alpha <= MG_ALPHA_MAX ? alpha * (m * X) : 0.f;  // no gradient through the active clamp
+            const float ddx = p.dx[k & 1], ddy = p.dy[k >> 1];
+            const float qx = q * ddx, qy = q * ddy;
+            S += q; Sx += qx; Sy += qy;
+            Sxx = fmaf(qx, ddx, Sxx);
+            Sxy = fmaf(qx, ddy, Sxy);
+            Syy = fmaf(qy, ddy, Syy);
           }
         }
       }
