@@ -94,21 +94,18 @@ __global__ void __launch_bounds__(RN_THREADS, RN_FWD_MINB) render_fwd_kernel(
               const float e = rn_eval(p, ra.w, k);
               const bool pass = rn_filter(e, lo) && ((live >> k) & 1u);
               if (__any_sync(0xffffffffu, pass)) {
-                if (pass) {
-                  const float alpha = fminf(MG_ALPHA_MAX, rn_ex2(e));
-                  const float a = m * alpha;
-                  const float Tn = T[k] * (1.f - a);
-                  if (Tn < MG_T_MIN) {
-                    live &= ~(1u << k);  // stop: this entry is not blended; pos - 1 entries were consumed
-                    last[k] = pos - 1;
-                  } else {
-                    const float w = a * T[k];
-                    Cr[k] = fmaf(w, rc.x, Cr[k]);
-                    Cg[k] = fmaf(w, rc.y, Cg[k]);
-                    Cb[k] = fmaf(w, rc.z, Cb[k]);
-                    T[k] = Tn;
-                  }
-                }
+                // branch-free inside the section: a pair that fails the filter blends with alpha = 0 (w = 0, T' = T)
+                const float alpha = pass ? fminf(MG_ALPHA_MAX, rn_ex2(e)) : 0.f;
+                const float a = m * alpha;
+                const float Tn = T[k] * (1.f - a);
+                const bool stop = pass && Tn < MG_T_MIN;  // this entry is not blended; pos - 1 entries were consumed
+                const float w = stop ? 0.f : a * T[k];
+                Cr[k] = fmaf(w, rc.x, Cr[k]);
+                Cg[k] = fmaf(w, rc.y, Cg[k]);
+                Cb[k] = fmaf(w, rc.z, Cb[k]);
+                T[k] = stop ? T[k] : Tn;
+                live = stop ? live & ~(1u << k) : live;
+                last[k] = stop ? pos - 1 : last[k];
               }
             }
           }
