@@ -173,8 +173,10 @@ __global__ void __launch_bounds__(RN_THREADS, RN_BWD_MINB) render_bwd_kernel(
       const int jj = 31 - __clz(todo);
       todo &= ~(1u << jj);
       const float4 ra = buf[jj].a, rb = buf[jj].b, rc = buf[jj].c;
-      const uint32_t sb = __float_as_uint(rc.w);
-      const float lo = rb.y, m = rb.z;
+      // the same record is read by every lane: a warp reduction hands the compiler that fact (uniform registers and
+      // branches for everything that depends on the sub-block mask and on M)
+      const uint32_t sb = __reduce_or_sync(0xffffffffu, __float_as_uint(rc.w));
+      const float lo = rb.y, m = __uint_as_float(__reduce_or_sync(0xffffffffu, __float_as_uint(rb.z)));
       const uint32_t pos = (uint32_t)(base + jj + 1);
       const RnPartial p = rn_partial(ra, rb, fx, fy);
 

@@ -83,7 +83,8 @@ __global__ void __launch_bounds__(RN_THREADS, RN_FWD_MINB) render_fwd_kernel(
         const int jj = __ffs(todo) - 1;
         todo &= todo - 1;
         const float4 ra = buf[jj].a, rb = buf[jj].b, rc = buf[jj].c;
-        const uint32_t sb = __float_as_uint(rc.w) & live_sb;
+        // the same record is read by every lane: a warp reduction hands the compiler that fact (uniform branches)
+        const uint32_t sb = __reduce_or_sync(0xffffffffu, __float_as_uint(rc.w)) & live_sb;
         const float lo = rb.y, m = rb.z;
         const uint32_t pos = (uint32_t)(base + jj + 1);
         const RnPartial p = rn_partial(ra, rb, fx, fy);
