@@ -33,7 +33,7 @@ FLOP_BLEND_FWD = 11   # per blend, forward
 FLOP_BLEND_BWD = 59   # per blend, backward (49 + 10 adds of the per-entry reduction)
 # dram__bytes_read.sum + dram__bytes_write.sum per launch at config 3, from the `ncu --set full` capture summarised
 # in profiles/r01z_final.md (the report itself is not committed); null for other configs
-NCU_TRAFFIC_BYTES = {3: {"render_bwd": 931.6e6 + 126.2e6, "render_fwd": 281.8e6 + 19.9e6}}
+NCU_TRAFFIC_BYTES = {3: {"render_bwd": 916.3e6 + 122.3e6, "render_fwd": 297.4e6 + 20.4e6}}
 # kernels of libmg launched per step (memsets and copies not counted): bin_sort = depth keys + ctl + 4 single-kernel
 # radix passes + row expansion (count, 2 scan, plan, emit) + column expansion (count, 2 scan, emit, ranges, tile order)
 KERNELS_PER_STEP = {"preprocess": 1, "bin_sort": 2 + 4 + 5 + 6, "render_fwd": 1, "render_bwd": 1,
