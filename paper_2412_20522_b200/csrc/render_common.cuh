@@ -103,30 +103,39 @@ __device__ __forceinline__ RnRecord rn_make_record(const RnRaw& v) {
   return r;
 }
 
-// Largest e over the pixel rectangle [xlo, xhi] x [ylo, yhi] (e is a concave quadratic in d; its
-// maximum over a box whose interior misses the centre lies on an edge next to the centre).
-__device__ __forceinline__ float rn_max_e_over_box(const float4& ra, const float4& rb, float xlo, float xhi, float ylo,
-                                                   float yhi) {
-  const float A2 = ra.z, B2 = ra.w, C2 = rb.x, lo = rb.y;
-  const float dxlo = ra.x - xhi, dxhi = ra.x - xlo;
-  const float dylo = ra.y - yhi, dyhi = ra.y - ylo;
-  const float dxc = fminf(fmaxf(0.f, dxlo), dxhi), dyc = fminf(fmaxf(0.f, dylo), dyhi);
-  // edge dx = dxc: best dy
-  const float dy1 = fminf(fmaxf(__fdividef(-B2 * dxc, 2.f * C2), dylo), dyhi);
-  const float e1 = lo + A2 * dxc * dxc + B2 * dxc * dy1 + C2 * dy1 * dy1;
-  // edge dy = dyc: best dx
-  const float dx2 = fminf(fmaxf(__fdividef(-B2 * dyc, 2.f * A2), dxlo), dxhi);
-  const float e2 = lo + A2 * dx2 * dx2 + B2 * dx2 * dyc + C2 * dyc * dyc;
-  return fmaxf(e1, e2);
-}
-
 // Bit k set = the entry can pass the alpha filter somewhere in sub-block k of the strip at (X0, Y0).
+// Per box: the largest e over the pixel rectangle (e is a concave quadratic in d; its maximum over a box whose
+// interior misses the centre lies on an edge next to the centre: the edge dx = dxc with the best dy, or the edge
+// dy = dyc with the best dx).  The four 8x4 boxes share their two x-intervals and two y-intervals, so everything that
+// depends on one axis only (clamped offsets, the unconstrained optimum along the other axis, the pure quadratic
+// terms) is computed twice, not four times; per box only the two clamps and the two edge values remain.
 __device__ __forceinline__ uint32_t rn_subblock_mask(const float4& ra, const float4& rb, float X0, float Y0) {
+  const float A2 = ra.z, B2 = ra.w, C2 = rb.x, lo = rb.y;
+  const float inv2C = __fdividef(1.f, 2.f * C2), inv2A = __fdividef(1.f, 2.f * A2);
+  float dxlo[2], dxhi[2], dxc[2], ty[2], qx[2], bx[2];  // per x-interval
+  float dylo[2], dyhi[2], dyc[2], tx[2], qy[2], by[2];  // per y-interval
+#pragma unroll
+  for (int i = 0; i < 2; i++) {
+    dxlo[i] = ra.x - (X0 + 8.f * i + 7.f); dxhi[i] = ra.x - (X0 + 8.f * i);
+    dxc[i] = fminf(fmaxf(0.f, dxlo[i]), dxhi[i]);
+    ty[i] = -B2 * dxc[i] * inv2C;       // best dy on the edge dx = dxc, before clamping
+    qx[i] = lo + A2 * dxc[i] * dxc[i];  // lo + A2 dxc^2
+    bx[i] = B2 * dxc[i];
+    dylo[i] = ra.y - (Y0 + 4.f * i + 3.f); dyhi[i] = ra.y - (Y0 + 4.f * i);
+    dyc[i] = fminf(fmaxf(0.f, dylo[i]), dyhi[i]);
+    tx[i] = -B2 * dyc[i] * inv2A;
+    qy[i] = lo + C2 * dyc[i] * dyc[i];
+    by[i] = B2 * dyc[i];
+  }
   uint32_t m = 0;
 #pragma unroll
   for (int k = 0; k < 4; k++) {
-    const float xlo = X0 + 8.f * (k & 1), ylo = Y0 + 4.f * (k >> 1);
-    if (rn_max_e_over_box(ra, rb, xlo, xlo + 7.f, ylo, ylo + 3.f) >= RN_LOG2_ALPHA_MIN - RN_CULL_SLACK) m |= 1u << k;
+    const int ix = k & 1, iy = k >> 1;
+    const float dy1 = fminf(fmaxf(ty[ix], dylo[iy]), dyhi[iy]);
+    const float e1 = qx[ix] + (bx[ix] + C2 * dy1) * dy1;
+    const float dx2 = fminf(fmaxf(tx[iy], dxlo[ix]), dxhi[ix]);
+    const float e2 = qy[iy] + (by[iy] + A2 * dx2) * dx2;
+    if (fmaxf(e1, e2) >= RN_LOG2_ALPHA_MIN - RN_CULL_SLACK) m |= 1u << k;
   }
   return m;
 }
