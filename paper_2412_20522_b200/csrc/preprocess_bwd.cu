@@ -83,9 +83,6 @@ __device__ __forceinline__ GeoGrads geometry_tail(const H* Rd, bool xcl, bool yc
 }
 
 constexpr int PB_THREADS = 128;
-#ifndef PB_MINB
-#define PB_MINB 4
-#endif
 #ifndef PB_G
 #define PB_G double
 #endif
