@@ -100,3 +100,28 @@ def test_constants_agree_between_header_and_oracle():
     for a, b in (("MG_TILE", "TILE"), ("MG_ALPHA_MIN", "ALPHA_MIN"), ("MG_ALPHA_MAX", "ALPHA_MAX"), ("MG_T_MIN", "T_MIN"),
                  ("MG_DILATION", "DILATION"), ("MG_ZNEAR", "ZNEAR"), ("MG_JCLAMP", "JCLAMP"), ("MG_EIG_FLOOR", "EIG_FLOOR")):
         assert abs(ev(hv(a)) - ev(ov(b))) < 1e-12, (a, hv(a), ov(b))
+
+
+def test_invalid_arguments_of_the_next_rows_are_rejected_without_a_gpu(lib):
+    """Mask head, compaction and render loss: argument checks happen before any CUDA call."""
+    from paper_2412_20522_b200 import binding
+
+    null = C.c_void_p(0)
+    rc = lib.mg_mask_sample(C.c_int64(10), null, null, C.c_float(0.0), null, null, null)
+    assert rc == binding.MG_ERR_INVALID_ARG and b"tau" in lib.mg_last_error_string()
+    rc = lib.mg_mask_sample(C.c_int64(10), null, null, C.c_float(1.0), null, null, null)
+    assert rc == binding.MG_ERR_INVALID_ARG and b"null" in lib.mg_last_error_string()
+    assert lib.mg_mask_sample(C.c_int64(0), null, null, C.c_float(1.0), null, null, null) == binding.MG_OK
+    rc = lib.mg_mask_sample_bwd(C.c_int64(-1), null, null, C.c_float(1.0), null, null)
+    assert rc == binding.MG_ERR_INVALID_ARG
+    rc = lib.mg_mask_loss(C.c_int64(0), null, C.c_float(0.1), null, null, null)
+    assert rc == binding.MG_ERR_INVALID_ARG  # the mean over zero Gaussians is undefined
+    rc = lib.mg_mask_prune_keep(C.c_int64(5), C.c_int32(-1), null, null, null, null)
+    assert rc == binding.MG_ERR_INVALID_ARG
+    assert binding.mg_compact_workspace_bytes(-1) == 0 and binding.mg_compact_workspace_bytes(1000) >= 4000
+    rc = lib.mg_compact(C.c_int64(10), null, C.c_int32(17), null, null, null, null, C.c_size_t(0), null, null)
+    assert rc == binding.MG_ERR_INVALID_ARG and b"n_arrays" in lib.mg_last_error_string()
+    assert binding.mg_render_loss_workspace_bytes(0, 5) == 0
+    assert binding.mg_render_loss_workspace_bytes(10, 5) == 9 * 4 * 50
+    rc = lib.mg_render_loss(C.c_int32(10), C.c_int32(5), null, null, C.c_float(0.2), null, null, null, C.c_size_t(0), null)
+    assert rc == binding.MG_ERR_INVALID_ARG
