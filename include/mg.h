@@ -18,6 +18,9 @@
  *     read during the call.  The caller owns every buffer; the library allocates nothing persistent.
  *   - `stream` is a cudaStream_t (NULL = default stream).  All work is enqueued on it; calls are
  *     asynchronous.
+ *     Calls may overlap on different streams as long as they share no buffer, with one exception:
+ *     mg_preprocess accumulates R in one device-side counter per device, so two mg_preprocess calls on the
+ *     same device must not run concurrently.
  *   - Layouts: packed row-major fp32.  means[N][3], log_scales[N][3], quats[N][4] as (w,x,y,z),
  *     opacity_logits[N], sh[N][K][3] with K=(sh_degree+1)^2 (coefficient-major, RGB innermost),
  *     masks[N] (any real value; tests use {0,1}; Eq. 4 is affine in M), images planar [3][H][W].

@@ -760,11 +760,13 @@ extern "C" int mg_bin_sort(const mg_camera* cam, int64_t N, const float* depths,
   }
 
   // S1: depth order of the N Gaussians (culled ones last), R, nvis, overflow flag, digit histograms
-  static int dk_grid = 0;
+  static int dk_grid_of[64] = {0};  // per device: function attributes and SM counts belong to a device
+  int dev = 0;
+  MG_CHECK_CUDA(cudaGetDevice(&dev));
+  int& dk_grid = dk_grid_of[dev & 63];
   if (dk_grid == 0) {
     MG_CHECK_CUDA(cudaFuncSetAttribute(radix_onesweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(RadixSmem)));
-    int dev = 0, sms = 0;
-    MG_CHECK_CUDA(cudaGetDevice(&dev));
+    int sms = 0;
     MG_CHECK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     dk_grid = sms * 8;
   }

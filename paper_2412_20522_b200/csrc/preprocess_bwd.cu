@@ -444,10 +444,12 @@ extern "C" int mg_preprocess_bwd(const mg_camera* cam, int64_t N, const float* m
   }
 #undef MG_LAUNCH
   MG_CHECK_LAUNCH();
-  static int geo_grid = 0;
+  static int geo_grid_of[64] = {0};  // per device
+  int dev = 0;
+  MG_CHECK_CUDA(cudaGetDevice(&dev));
+  int& geo_grid = geo_grid_of[dev & 63];
   if (geo_grid == 0) {
-    int dev = 0, sms = 0;
-    MG_CHECK_CUDA(cudaGetDevice(&dev));
+    int sms = 0;
     MG_CHECK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     geo_grid = 2 * sms;
   }

@@ -158,7 +158,10 @@ extern "C" int mg_render_loss(int32_t width, int32_t height, const float* image,
     return MG_ERR_CAPACITY;
   }
   cudaStream_t st = (cudaStream_t)stream;
-  static bool win_set = false;
+  static bool win_set_of[64] = {false};  // per device: __constant__ memory belongs to a device
+  int dev = 0;
+  MG_CHECK_CUDA(cudaGetDevice(&dev));
+  bool& win_set = win_set_of[dev & 63];
   if (!win_set) {
     double g[2 * RL_R + 1], sum = 0.0;
     for (int k = 0; k <= 2 * RL_R; k++) { const double x = k - RL_R; g[k] = exp(-(x * x) / (2.0 * 1.5 * 1.5)); sum += g[k]; }
