@@ -14,7 +14,8 @@ constexpr int MH_THREADS = 256;
 
 // d = (s_1 + g_1) - (s_0 + g_0) with g = -log(-log u): the hard sample is d > 0, the soft one sigmoid(d / tau).
 __device__ __forceinline__ float perturbed_gap(float2 s, float2 u) {
-  const float g0 = -logf(-logf(u.x)), g1 = -logf(-logf(u.y));
+  // inner log accurate (for u near 1, -log u is tiny and needs its relative accuracy), outer log lg2-based
+  const float g0 = -__logf(-logf(u.x)), g1 = -__logf(-logf(u.y));
   return (s.y + g1) - (s.x + g0);
 }
 
