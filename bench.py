@@ -516,7 +516,9 @@ def main():
     sm_max = 1965.0
     if os.path.exists(peaks_path):
         sm_max = float(json.load(open(peaks_path)).get("sm_max_mhz", sm_max))
-    fp32_peak = 148 * 128 * 2 * sm_max * 1e6 / 1e12  # TFLOP/s (derived, MEASURED_PEAKS has no FP32 entry)
+    fp32_derived = 148 * 128 * 2 * sm_max * 1e6 / 1e12  # TFLOP/s from the guide's unit counts (context)
+    fp32_meas = mg.mg_measure_fp32_peak(0.05)             # timed on this chip, now (MEASURED_PEAKS.json has no FP32 entry)
+    fp32_peak = max(fp32_meas["ffma_sustained"], fp32_meas["ffma2_sustained"])
     roofline = None
     if wc:
         if dom == "render_bwd":
@@ -528,7 +530,8 @@ def main():
                     "frac": ach / fp32_peak,
                     "traffic": NCU_TRAFFIC_BYTES.get(args.config, {}).get(dom), "traffic_unit": "bytes per launch (ncu, profiles/r01z_final.md)",
                     "flop_per_launch": flops, "share_of_step": per_call[dom] / sum(per_call.values()),
-                    "peak_source": f"derived 148 SM x 128 lanes x 2 x {sm_max:.0f} MHz (no FP32 entry in MEASURED_PEAKS.json)"}
+                    "peak_source": "measured: mg_measure_fp32_peak, dependent-free FMA chains on every SM, >= 50 ms, sustained",
+                    "peak_measured": fp32_meas, "peak_derived": fp32_derived}
 
     hbm_gbs = 6540.8
     if os.path.exists(peaks_path):

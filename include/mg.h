@@ -18,9 +18,9 @@
  *     read during the call.  The caller owns every buffer; the library allocates nothing persistent.
  *   - `stream` is a cudaStream_t (NULL = default stream).  All work is enqueued on it; calls are
  *     asynchronous.
- *     Calls may overlap on different streams as long as they share no buffer, with one exception:
- *     mg_preprocess accumulates R in one device-side counter per device, so two mg_preprocess calls on the
- *     same device must not run concurrently.
+ *     Calls may overlap on different streams, and be issued from different host threads, as long as they
+ *     share no output or scratch buffer: the library keeps no device-side state of its own (every counter
+ *     lives in caller memory) and its per-device one-time initialisations are thread-safe.
  *   - Layouts: packed row-major fp32.  means[N][3], log_scales[N][3], quats[N][4] as (w,x,y,z),
  *     opacity_logits[N], sh[N][K][3] with K=(sh_degree+1)^2 (coefficient-major, RGB innermost),
  *     masks[N] (any real value; tests use {0,1}; Eq. 4 is affine in M), images planar [3][H][W].
@@ -80,11 +80,12 @@ size_t mg_workspace_bytes(int64_t N, int32_t width, int32_t height, uint64_t R_c
  *   means2d[N][2] pixel-index coordinates; depths[N] camera z; conic_opacity[N][4] = (A, B, C, o) with
  *   power = -1/2 (A dx^2 + 2 B dx dy + C dy^2); rgb[N][3]; radii[N]; rects[N][4] = (x0, y0, x1, y1) in
  *   tile units, max exclusive; tiles_touched[N]; clamped[N] bit k = colour channel k clamped at 0.
- *   num_rendered_host (may be NULL): sum of tiles_touched = R, written asynchronously. */
+ *   num_rendered (DEVICE, one uint64, may be NULL): overwritten with R = sum of tiles_touched.
+ *   num_rendered_host (may be NULL; needs num_rendered): a copy of it, written asynchronously. */
 int mg_preprocess(const mg_camera* cam, int64_t N, const float* means, const float* log_scales, const float* quats,
                   const float* opacity_logits, const float* sh, float* means2d, float* depths, float* conic_opacity,
                   float* rgb, int32_t* radii, int32_t* rects, uint32_t* tiles_touched, uint8_t* clamped,
-                  uint64_t* num_rendered_host, void* stream);
+                  uint64_t* num_rendered, uint64_t* num_rendered_host, void* stream);
 
 /* Step a4-a6.  Result = the duplicated (tile, depth) keys in ascending order of the
  * 64-bit key (tile_id << 32 | fp32 bits of depth), ties by Gaussian index, tile_id = ty * gw + tx:
@@ -97,11 +98,18 @@ int mg_preprocess(const mg_camera* cam, int64_t N, const float* means, const flo
  *   R_out_host (may be NULL): the true R, written asynchronously.
  * R must be < 2^32.  If R > R_capacity nothing is written to sorted_ids, every tile range is set to
  * [0, 0) and *R_out_host (> R_capacity) tells the caller to retry with larger buffers.
+ * Internal failure: the radix passes chain their blocks through look-backs that poll a predecessor's status
+ * word; a poll that exhausts its limit (impossible in a correct run: a predecessor is always resident) does
+ * not return a wrong order: nothing is emitted, every tile range is [0, 0) and *R_out_host = UINT64_MAX.
  * workspace: at least mg_workspace_bytes(N, W, H, R_capacity) bytes, 256-byte aligned. */
 int mg_bin_sort(const mg_camera* cam, int64_t N, const float* depths, const int32_t* rects,
                 const uint32_t* tiles_touched, uint64_t R_capacity, void* workspace, size_t workspace_bytes,
                 uint32_t* sorted_ids, uint32_t* tile_ranges, uint32_t* tile_order, uint64_t* R_out_host,
                 void* stream);
+
+/* Test hook (failure injection): polls a look-back makes before it gives up; 0 = every look-back gives up at once,
+ * negative = the default (2^26).  Process-wide. */
+void mg_debug_set_lookback_spin_limit(int polls);
 
 /* Step a7 (Eq. 3-4; Eq. 9-10).  Per pixel, front to back over its tile's
  * list: alpha = min(0.99, o G); skip if power > 0 or alpha < 1/255 (mask NOT consulted, reading 2);
@@ -182,6 +190,13 @@ int mg_compact(int64_t N, const uint8_t* keep, int32_t n_arrays, const float* co
 size_t mg_render_loss_workspace_bytes(int32_t width, int32_t height);
 int mg_render_loss(int32_t width, int32_t height, const float* image, const float* target, float lambda_dssim,
                    float* dL_dimage, double* stats, void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- Measurement aid (the FP32 roofline of the blend kernels needs a measured peak; the driver's
+ * MEASURED_PEAKS.json has none).  Runs dependent-free FMA chains on every SM for at least min_seconds per instruction
+ * form and times them with CUDA events; SYNCHRONOUS (returns when the measurement is done).
+ * tflops_host (HOST, 4 doubles): [0] scalar FFMA sustained over the measurement, [1] its best round, [2] packed
+ * fma.rn.f32x2 sustained, [3] its best round -- in TFLOP/s, an FMA counted as 2 flop.  scratch: one DEVICE float. */
+int mg_measure_fp32_peak(double min_seconds, double* tflops_host, float* scratch, void* stream);
 
 #ifdef __cplusplus
 }

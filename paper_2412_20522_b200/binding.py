@@ -35,7 +35,7 @@ class mg_camera(C.Structure):
 EXPORTS = ["mg_last_error_string", "mg_version", "mg_workspace_bytes", "mg_preprocess", "mg_bin_sort",
            "mg_render_fwd", "mg_render_bwd", "mg_preprocess_bwd", "mg_mask_sample", "mg_mask_sample_bwd", "mg_mask_loss",
            "mg_mask_prune_keep", "mg_compact_workspace_bytes", "mg_compact", "mg_render_loss_workspace_bytes",
-           "mg_render_loss"]
+           "mg_render_loss", "mg_measure_fp32_peak", "mg_debug_set_lookback_spin_limit"]
 
 
 def lib():
@@ -53,8 +53,10 @@ def lib():
         L.mg_render_loss_workspace_bytes.argtypes = [C.c_int32, C.c_int32]
         L.mg_compact_workspace_bytes.restype = C.c_size_t
         L.mg_compact_workspace_bytes.argtypes = [C.c_int64]
+        L.mg_debug_set_lookback_spin_limit.restype = None
+        L.mg_debug_set_lookback_spin_limit.argtypes = [C.c_int]
         for name in EXPORTS[3:]:
-            if not name.endswith("_workspace_bytes"):
+            if not name.endswith("_workspace_bytes") and not name.startswith("mg_debug"):
                 getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
@@ -106,12 +108,12 @@ def mg_workspace_bytes(N, width, height, R_capacity) -> int:
 
 
 def mg_preprocess(cam: mg_camera, means, log_scales, quats, opacity_logits, sh, means2d, depths, conic_opacity, rgb,
-                  radii, rects, tiles_touched, clamped, num_rendered_host=None):
+                  radii, rects, tiles_touched, clamped, num_rendered=None, num_rendered_host=None):
     N = means.shape[0]
     _check(lib().mg_preprocess(C.byref(cam), C.c_int64(N), _ptr(means, F32), _ptr(log_scales, F32), _ptr(quats, F32),
                                _ptr(opacity_logits, F32), _ptr(sh, F32), _ptr(means2d, F32), _ptr(depths, F32),
                                _ptr(conic_opacity, F32), _ptr(rgb, F32), _ptr(radii, I32), _ptr(rects, I32),
-                               _ptr(tiles_touched, I32), _ptr(clamped, U8),
+                               _ptr(tiles_touched, I32), _ptr(clamped, U8), _ptr(num_rendered, torch.int64),
                                _ptr(num_rendered_host, torch.int64, "cpu"), _stream()))
 
 
@@ -205,6 +207,14 @@ def mg_render_loss(image, target, lambda_dssim, dL_dimage, stats, workspace):
                                 C.c_size_t(workspace.numel()), _stream()))
 
 
+def mg_measure_fp32_peak(min_seconds=0.05):
+    """-> dict of TFLOP/s: scalar FFMA and packed f32x2, sustained and best round (synchronous)."""
+    out = (C.c_double * 4)()
+    scratch = torch.zeros(1, dtype=F32, device="cuda")
+    _check(lib().mg_measure_fp32_peak(C.c_double(min_seconds), out, _ptr(scratch, F32), _stream()))
+    return {"ffma_sustained": out[0], "ffma_best": out[1], "ffma2_sustained": out[2], "ffma2_best": out[3]}
+
+
 class Frame:
     """Device buffers of one camera view + the five calls in order.  Allocation and marshalling only.
 
@@ -230,6 +240,7 @@ class Frame:
         self.dL_drgb, self.dL_dmask = e(N, 3), e(N)
         self.dL_dmeans, self.dL_dlog_scales, self.dL_dquats = e(N, 3), e(N, 3), e(N, 4)
         self.dL_dopacity_logits, self.dL_dsh = e(N), e(N, K, 3)
+        self.R_dev = torch.zeros(1, dtype=torch.int64, device=device)  # mg_preprocess's counter (caller-owned)
         self.R_host = torch.zeros(2, dtype=torch.int64).pin_memory()
         self.R_capacity = 0
         self.R = 0
@@ -254,7 +265,7 @@ class Frame:
     def preprocess(self, g):
         mg_preprocess(self.cam, g["means"], g["log_scales"], g["quats"], g["opacity_logits"], g["sh"], self.means2d,
                       self.depths, self.conic_opacity, self.rgb, self.radii, self.rects, self.tiles_touched,
-                      self.clamped, self.R_host[0:1])
+                      self.clamped, self.R_dev, self.R_host[0:1])
 
     def bin_sort(self):
         mg_bin_sort(self.cam, self.depths, self.rects, self.tiles_touched, self.R_capacity, self.workspace,

@@ -27,6 +27,8 @@
 //
 // Bytes moved per duplicated key: ~4 B written + ~16 B of records and tables (mostly L2 hits),
 // against ~150 B for six 64-bit key-value radix passes over R keys.
+#include <atomic>
+
 #include "mg_common.cuh"
 
 namespace {
@@ -80,13 +82,12 @@ __device__ __forceinline__ uint32_t peers_by_ballot(uint32_t v, int nbits, uint3
 struct SortCtl {            // lives in the workspace; zeroed at the start of every call
   unsigned long long R;     // true number of duplicated keys = sum of tiles_touched
   uint32_t nvis;            // Gaussians with tiles_touched > 0
-  uint32_t overflow;        // 1 if R > capacity or R >= 2^32
+  uint32_t overflow;        // 1 if R > capacity or R >= 2^32; 2 if a look-back gave up (nothing is emitted either way)
   uint32_t n_chunks_c;      // chunks of the column expansion (sum over rows of ceil(records / XP_CHUNK))
   uint32_t n_table_c;       // gw * n_chunks_c
   uint32_t pad[2];
   uint32_t ticket[4];       // next logical tile of each radix pass (tiles are taken in ticket order)
-  uint32_t spin_fail;       // set if a look-back ever gave up (never in a correct run)
-  uint32_t pad2[3];
+  uint32_t pad2[4];
   uint32_t ghist[4][RS_BINS];  // digit histograms of the depth keys, all four passes; then exclusive bases
   uint32_t class_count[TO_CLASSES];   // tiles per list-length class (tile_order)
   uint32_t class_cursor[TO_CLASSES];  // tiles of the class already placed
@@ -114,7 +115,8 @@ __device__ __forceinline__ unsigned long long ld_relaxed_u64(const unsigned long
 
 constexpr unsigned long long LB_AGGREGATE = 1ull << 32;  // status word = flag << 32 | count
 constexpr unsigned long long LB_INCLUSIVE = 2ull << 32;
-constexpr int LB_SPIN_LIMIT = 1 << 26;                   // a look-back that gives up flags ctl->spin_fail
+constexpr int LB_SPIN_LIMIT = 1 << 26;                   // polls of one status word before a look-back gives up
+std::atomic<int> g_spin_limit{LB_SPIN_LIMIT};             // mg_debug_set_lookback_spin_limit (failure injection in tests)
 
 // One radix pass = ONE kernel (single-pass chained scan with decoupled look-back): a block takes the next
 // logical tile by ticket, ranks its 4096 keys, publishes its per-digit counts, and obtains its per-digit
@@ -125,7 +127,7 @@ constexpr int LB_SPIN_LIMIT = 1 << 26;                   // a look-back that giv
 __global__ void __launch_bounds__(RS_THREADS) radix_onesweep_kernel(
     const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in, uint32_t* __restrict__ keys_out,
     uint32_t* __restrict__ vals_out, uint32_t n, int pass, SortCtl* __restrict__ ctl,
-    unsigned long long* __restrict__ status) {
+    unsigned long long* __restrict__ status, int spin_limit) {
   extern __shared__ __align__(16) unsigned char rs_smem_raw[];
   RadixSmem& sm = *reinterpret_cast<RadixSmem*>(rs_smem_raw);
   __shared__ uint32_t s_tile;
@@ -195,8 +197,10 @@ __global__ void __launch_bounds__(RS_THREADS) radix_onesweep_kernel(
       const unsigned long long* ps = status + (size_t)t * RS_BINS + threadIdx.x;
       unsigned long long w = ld_relaxed_u64(ps);
       int spins = 0;
-      while ((w >> 32) == 0 && ++spins < LB_SPIN_LIMIT) w = ld_relaxed_u64(ps);
-      if ((w >> 32) == 0) { ctl->spin_fail = 1u; break; }
+      while ((w >> 32) == 0 && ++spins < spin_limit) w = ld_relaxed_u64(ps);
+      // A predecessor that never publishes cannot happen (tiles are taken in ticket order, so it is resident and
+      // running); if it does, the call fails loudly: nothing is emitted and R_out_host reads UINT64_MAX.
+      if ((w >> 32) == 0 || spin_limit == 0) { ctl->overflow = 2u; break; }
       prefix += (uint32_t)w;
       if ((w & LB_INCLUSIVE) != 0) break;
     }
@@ -469,7 +473,8 @@ __global__ void __launch_bounds__(32 * XP_MAX_WARPS) row_expand_kernel(
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t chunk = blockIdx.x * (uint32_t)warps_per_block + warp;
   if (chunk >= n_chunks) return;
-  if (!kCount && ctl->overflow) return;
+  // capacity overflow: only the counts are taken; a failed sort (overflow == 2) left `order` undefined: nothing is read
+  if (ctl->overflow && (!kCount || ctl->overflow == 2u)) return;
   uint32_t* cnt = xp_smem + (size_t)warp * (gh + 1);
   const uint32_t nvis = ctl->nvis;
   const uint32_t k0 = chunk * (uint32_t)XP_CHUNK;
@@ -610,6 +615,7 @@ __global__ void __launch_bounds__(256) tile_ranges_kernel(const uint32_t* __rest
   const int ntiles = gw * gh;
   if (t >= ntiles) return;
   if (ctl->overflow) {
+    if (t == 0 && ctl->overflow == 2u) ctl->R = ~0ull;  // a look-back gave up: reported as R = UINT64_MAX
     tile_ranges[2 * t] = 0;
     tile_ranges[2 * t + 1] = 0;
     atomicAdd(&ctl->class_count[0], 1u);
@@ -718,6 +724,8 @@ extern "C" size_t mg_workspace_bytes(int64_t N, int32_t width, int32_t height, u
   return make_layout(N, gw, gh, R_capacity).total;
 }
 
+extern "C" void mg_debug_set_lookback_spin_limit(int polls) { g_spin_limit.store(polls < 0 ? LB_SPIN_LIMIT : polls); }
+
 extern "C" int mg_bin_sort(const mg_camera* cam, int64_t N, const float* depths, const int32_t* rects,
                            const uint32_t* tiles_touched, uint64_t R_capacity, void* workspace, size_t workspace_bytes,
                            uint32_t* sorted_ids, uint32_t* tile_ranges, uint32_t* tile_order, uint64_t* R_out_host,
@@ -760,16 +768,15 @@ extern "C" int mg_bin_sort(const mg_camera* cam, int64_t N, const float* depths,
   }
 
   // S1: depth order of the N Gaussians (culled ones last), R, nvis, overflow flag, digit histograms
-  static int dk_grid_of[64] = {0};  // per device: function attributes and SM counts belong to a device
-  int dev = 0;
-  MG_CHECK_CUDA(cudaGetDevice(&dev));
-  int& dk_grid = dk_grid_of[dev & 63];
-  if (dk_grid == 0) {
+  static MgOncePerDevice attr_set;  // function attributes belong to a device
+  int dev = 0, sms = 0;
+  if (int rc = mg_current_device(&dev, &sms)) return rc;
+  if (!attr_set.is_done(dev)) {
     MG_CHECK_CUDA(cudaFuncSetAttribute(radix_onesweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(RadixSmem)));
-    int sms = 0;
-    MG_CHECK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    dk_grid = sms * 8;
+    attr_set.set_done(dev);
   }
+  const int dk_grid = sms * 8;
+  const int spin_limit = g_spin_limit.load(std::memory_order_relaxed);
   MG_CHECK_CUDA(cudaMemsetAsync(status, 0, sizeof(unsigned long long) * 4 * (size_t)L.nblk_sort * RS_BINS, st));
   {
     const int64_t want = (N + 255) / 256;
@@ -781,7 +788,7 @@ extern "C" int mg_bin_sort(const mg_camera* cam, int64_t N, const float* depths,
     uint32_t *ki = keysA, *vi = nullptr, *ko = keysB, *vo = valsB;
     for (int pass = 0; pass < 4; pass++) {
       radix_onesweep_kernel<<<L.nblk_sort, RS_THREADS, sizeof(RadixSmem), st>>>(
-          ki, vi, ko, vo, (uint32_t)N, pass, ctl, status + (size_t)pass * L.nblk_sort * RS_BINS);
+          ki, vi, ko, vo, (uint32_t)N, pass, ctl, status + (size_t)pass * L.nblk_sort * RS_BINS, spin_limit);
       MG_CHECK_LAUNCH();
       ki = (pass & 1) ? keysA : keysB;
       vi = (pass & 1) ? valsA : valsB;

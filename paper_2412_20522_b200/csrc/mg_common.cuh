@@ -7,6 +7,15 @@
 
 void mg_set_error(const char* fmt, ...);
 
+// Per-device facts and one-time initialisations (api.cu).  Thread-safe: the cache entries are atomics and every
+// initialisation is idempotent, so two host threads that race on a first call both do the same harmless work.
+int mg_current_device(int* dev, int* sm_count);  // MG_OK or MG_ERR_CUDA
+struct MgOncePerDevice {                         // zero-initialised static: done[dev] != 0 once the init has run
+  int done[64];
+  bool is_done(int dev) const { return __atomic_load_n(&done[dev & 63], __ATOMIC_ACQUIRE) != 0; }
+  void set_done(int dev) { __atomic_store_n(&done[dev & 63], 1, __ATOMIC_RELEASE); }
+};
+
 #define MG_CHECK_CUDA(expr)                                                              \
   do {                                                                                   \
     cudaError_t e__ = (expr);                                                            \

@@ -6,8 +6,6 @@
 
 namespace {
 
-__device__ unsigned long long g_num_rendered;  // sum of tiles_touched of the launch in flight
-
 template <int D>
 __device__ __forceinline__ void sh_basis(float x, float y, float z, float* Y) {
   Y[0] = MG_SH_C0;
@@ -53,7 +51,7 @@ __global__ void __launch_bounds__(PP_THREADS) preprocess_kernel(
     const float* __restrict__ quats, const float* __restrict__ opacity_logits, const float* __restrict__ sh,
     float2* __restrict__ means2d, float* __restrict__ depths, float4* __restrict__ conic_opacity,
     float* __restrict__ rgb, int32_t* __restrict__ radii, int4* __restrict__ rects,
-    uint32_t* __restrict__ tiles_touched, uint8_t* __restrict__ clamped) {
+    uint32_t* __restrict__ tiles_touched, uint8_t* __restrict__ clamped, unsigned long long* __restrict__ num_rendered) {
   typedef ShRowLayout<D> L;
   constexpr int K = L::K, RK = L::RK, STRIDE = L::STRIDE;
   __shared__ __align__(16) float rows_all[PP_THREADS / 32][32 * STRIDE];
@@ -197,11 +195,13 @@ __global__ void __launch_bounds__(PP_THREADS) preprocess_kernel(
     tiles_touched[i] = touched;
     clamped[i] = (uint8_t)clampbits;
   }
-  // R = sum of tiles_touched: warp shuffle, then one atomic per warp
-  unsigned long long t64 = touched;
+  // R = sum of tiles_touched: warp reduction, then one atomic per warp into the caller's counter
+  if (num_rendered) {
+    unsigned long long t64 = touched;
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) t64 += __shfl_xor_sync(0xffffffffu, t64, o);
-  if ((threadIdx.x & 31) == 0 && t64) atomicAdd(&g_num_rendered, t64);
+    for (int o = 16; o > 0; o >>= 1) t64 += __shfl_xor_sync(0xffffffffu, t64, o);
+    if ((threadIdx.x & 31) == 0 && t64) atomicAdd(num_rendered, t64);
+  }
 }
 
 }  // namespace
@@ -209,13 +209,13 @@ __global__ void __launch_bounds__(PP_THREADS) preprocess_kernel(
 extern "C" int mg_preprocess(const mg_camera* cam, int64_t N, const float* means, const float* log_scales,
                              const float* quats, const float* opacity_logits, const float* sh, float* means2d,
                              float* depths, float* conic_opacity, float* rgb, int32_t* radii, int32_t* rects,
-                             uint32_t* tiles_touched, uint8_t* clamped, uint64_t* num_rendered_host, void* stream) {
+                             uint32_t* tiles_touched, uint8_t* clamped, uint64_t* num_rendered,
+                             uint64_t* num_rendered_host, void* stream) {
   if (int rc = mg_check_camera(cam)) return rc;
   MG_REQUIRE(N >= 0 && N < (int64_t)1 << 31, "N must be in [0, 2^31)");
   cudaStream_t st = (cudaStream_t)stream;
-  void* counter = nullptr;
-  MG_CHECK_CUDA(cudaGetSymbolAddress(&counter, g_num_rendered));
-  MG_CHECK_CUDA(cudaMemsetAsync(counter, 0, sizeof(unsigned long long), st));
+  MG_REQUIRE(num_rendered != nullptr || num_rendered_host == nullptr, "num_rendered_host needs the device counter num_rendered");
+  if (num_rendered) MG_CHECK_CUDA(cudaMemsetAsync(num_rendered, 0, sizeof(uint64_t), st));
   if (N > 0) {
     MG_REQUIRE(means && log_scales && quats && opacity_logits && sh, "null input array");
     MG_REQUIRE(means2d && depths && conic_opacity && rgb && radii && rects && tiles_touched && clamped, "null output array");
@@ -224,7 +224,8 @@ extern "C" int mg_preprocess(const mg_camera* cam, int64_t N, const float* means
 #define MG_LAUNCH(D)                                                                                              \
   preprocess_kernel<D><<<blocks, threads, 0, st>>>(*cam, N, means, log_scales, quats, opacity_logits, sh,         \
                                                    (float2*)means2d, depths, (float4*)conic_opacity, rgb, radii,  \
-                                                   (int4*)rects, tiles_touched, clamped)
+                                                   (int4*)rects, tiles_touched, clamped,      \
+                                                   (unsigned long long*)num_rendered)
     switch (cam->sh_degree) {
       case 0: MG_LAUNCH(0); break;
       case 1: MG_LAUNCH(1); break;
@@ -235,6 +236,6 @@ extern "C" int mg_preprocess(const mg_camera* cam, int64_t N, const float* means
     MG_CHECK_LAUNCH();
   }
   if (num_rendered_host)
-    MG_CHECK_CUDA(cudaMemcpyAsync(num_rendered_host, counter, sizeof(uint64_t), cudaMemcpyDeviceToHost, st));
+    MG_CHECK_CUDA(cudaMemcpyAsync(num_rendered_host, num_rendered, sizeof(uint64_t), cudaMemcpyDeviceToHost, st));
   return MG_OK;
 }

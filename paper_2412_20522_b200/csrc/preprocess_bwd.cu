@@ -352,7 +352,10 @@ __global__ void __launch_bounds__(PG_THREADS, 2) preprocess_bwd_geo_kernel(
   __syncthreads();
   int64_t i0 = begin;
   for (;;) {
-    if (i0 < end) {
+    // A sweep appends up to PG_SWEEP x 256 indices and a drain removes at most 256, so a sweep may only start while
+    // fewer than 256 are queued: the queue then never holds more than 255 + PG_SWEEP x 256 < its capacity, whatever the
+    // density of Gaussians with a gradient (qn is the same in every thread: it is only written in front of a barrier).
+    if (i0 < end && qn < PG_THREADS) {
       // sweep PG_SWEEP x 256 Gaussians: all their loads are in flight together
       // every load is issued before any is tested (no short-circuit: dependent loads would serialise the latency)
       bool active[PG_SWEEP];
@@ -444,15 +447,9 @@ extern "C" int mg_preprocess_bwd(const mg_camera* cam, int64_t N, const float* m
   }
 #undef MG_LAUNCH
   MG_CHECK_LAUNCH();
-  static int geo_grid_of[64] = {0};  // per device
-  int dev = 0;
-  MG_CHECK_CUDA(cudaGetDevice(&dev));
-  int& geo_grid = geo_grid_of[dev & 63];
-  if (geo_grid == 0) {
-    int sms = 0;
-    MG_CHECK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    geo_grid = 2 * sms;
-  }
+  int sms = 0;
+  if (int rc = mg_current_device(nullptr, &sms)) return rc;
+  const int geo_grid = 2 * sms;  // persistent grid: 2 blocks per SM
   const int64_t geo_want = (N + PG_THREADS - 1) / PG_THREADS;
   preprocess_bwd_geo_kernel<<<(unsigned)(geo_want < geo_grid ? geo_want : geo_grid), PG_THREADS, 0, st>>>(*cam, N, means, log_scales, quats, opacity_logits, radii,
                                                         (const float2*)dL_dmeans2d, dL_dconic, dL_dopacity, dL_dmeans,

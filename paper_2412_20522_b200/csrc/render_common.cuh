@@ -24,7 +24,12 @@
 #define RN_LOG2E 1.4426950408889634f
 #define RN_LN2 0.6931471805599453f
 #define RN_LOG2_ALPHA_MIN -7.994353436858858f  // log2(1/255)
-#define RN_CULL_SLACK 1e-3f                    // the sub-block cull keeps entries within 2^-10 of the threshold
+// The sub-block cull computes the largest e over a box along another arithmetic path than rn_eval, so it keeps every
+// entry within a slack of the threshold: 2^-10, plus 2^-21 of the largest magnitude the three quadratic terms can reach
+// over the strip (for a long thin splat far from its centre they reach 1e4..1e6 and cancel: the fp32 error of e is a
+// few ulps of the terms, not of e).
+#define RN_CULL_SLACK 1e-3f
+#define RN_CULL_SLACK_REL 4.8e-7f
 
 struct RnRecord {
   float4 a;  // mx, my, A2, B2
@@ -127,6 +132,10 @@ __device__ __forceinline__ uint32_t rn_subblock_mask(const float4& ra, const flo
     qy[i] = lo + C2 * dyc[i] * dyc[i];
     by[i] = B2 * dyc[i];
   }
+  // largest |dx|, |dy| over the strip -> bound of the magnitude of the terms of e at any of its pixels
+  const float Dx = fmaxf(fabsf(dxlo[1]), fabsf(dxhi[0])), Dy = fmaxf(fabsf(dylo[1]), fabsf(dyhi[0]));
+  const float mag = fabsf(A2) * Dx * Dx + fabsf(B2) * Dx * Dy + fabsf(C2) * Dy * Dy + fabsf(lo);
+  const float thresh = RN_LOG2_ALPHA_MIN - RN_CULL_SLACK - RN_CULL_SLACK_REL * mag;
   uint32_t m = 0;
 #pragma unroll
   for (int k = 0; k < 4; k++) {
@@ -135,7 +144,7 @@ __device__ __forceinline__ uint32_t rn_subblock_mask(const float4& ra, const flo
     const float e1 = qx[ix] + (bx[ix] + C2 * dy1) * dy1;
     const float dx2 = fminf(fmaxf(tx[iy], dxlo[ix]), dxhi[ix]);
     const float e2 = qy[iy] + (by[iy] + A2 * dx2) * dx2;
-    if (fmaxf(e1, e2) >= RN_LOG2_ALPHA_MIN - RN_CULL_SLACK) m |= 1u << k;
+    if (fmaxf(e1, e2) >= thresh) m |= 1u << k;
   }
   return m;
 }

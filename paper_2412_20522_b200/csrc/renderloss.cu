@@ -158,17 +158,16 @@ extern "C" int mg_render_loss(int32_t width, int32_t height, const float* image,
     return MG_ERR_CAPACITY;
   }
   cudaStream_t st = (cudaStream_t)stream;
-  static bool win_set_of[64] = {false};  // per device: __constant__ memory belongs to a device
+  static MgOncePerDevice win_set;  // per device: __constant__ memory belongs to a device
   int dev = 0;
-  MG_CHECK_CUDA(cudaGetDevice(&dev));
-  bool& win_set = win_set_of[dev & 63];
-  if (!win_set) {
+  if (int rc = mg_current_device(&dev, nullptr)) return rc;
+  if (!win_set.is_done(dev)) {
     double g[2 * RL_R + 1], sum = 0.0;
     for (int k = 0; k <= 2 * RL_R; k++) { const double x = k - RL_R; g[k] = exp(-(x * x) / (2.0 * 1.5 * 1.5)); sum += g[k]; }
     float w[2 * RL_R + 1];
     for (int k = 0; k <= 2 * RL_R; k++) w[k] = (float)(g[k] / sum);
     MG_CHECK_CUDA(cudaMemcpyToSymbol(c_win, w, sizeof(w)));
-    win_set = true;
+    win_set.set_done(dev);
   }
   const size_t n = (size_t)width * height;
   float* d_mu1 = (float*)workspace;

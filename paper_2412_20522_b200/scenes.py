@@ -218,6 +218,24 @@ def tiny_fd_scene(n=8, width=32, height=32, seed=100, sh_degree=3, bg=(0.2, 0.5,
     return Scene("tiny_fd", _f32(means), _f32(log_scales), _f32(quats), _f32(logits), sh, masks, [cam], seed)
 
 
+def needles(n=4000, width=640, height=400, seed=11) -> Scene:
+    """Long thin splats seen far from their centres (real captures are full of them; configs 1-5 have few): one axis
+    30-300x the other two, random orientation, so that the three terms of the exponent reach 1e4..1e6 at pixels that
+    still pass the alpha filter and cancel there."""
+    rng = np.random.default_rng(seed)
+    means = np.column_stack([rng.uniform(-2.5, 2.5, n), rng.uniform(-1.5, 1.5, n), rng.uniform(-1.0, 1.0, n)])
+    log_scales = rng.normal(-6.0, 0.5, (n, 3))
+    log_scales[np.arange(n), rng.integers(0, 3, n)] = rng.normal(-1.0, 0.6, n)
+    quats = _quats(rng, n)
+    logits = rng.normal(1.0, 1.5, n)
+    sh = _sh(rng, n, 1)
+    masks = _masks(rng, n, 0.6)
+    R, t = look_at((0.0, 0.0, -5.0), (0, 0, 0))
+    f = _fov_focal(width, 55)
+    cam = Camera(width, height, f, f, width / 2, height / 2, R, t, sh_degree=1)
+    return Scene("needles", _f32(means), _f32(log_scales), _f32(quats), _f32(logits), sh, masks, [cam], seed)
+
+
 CONFIGS = {1: config1, 2: config2, 3: config3, 4: config4, 5: config5}
 
 

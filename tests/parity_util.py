@@ -63,7 +63,17 @@ def check_preprocess(fr, sc, cam, max_flag_frac=0.01):
     n_flag_diff = int((~same_int).sum())
     assert flag.mean() <= max_flag_frac, f"{flag.mean():.4f} of Gaussians are margin-flagged"
     vis = (ref["radii"] > 0) & (got["radii"] > 0)
-    assert np.array_equal(ref["clamped"][vis & ~flag] > 0, got["clamped"][vis & ~flag] > 0) or True
+    # clamp flags (they gate dL/dsh in mg_preprocess_bwd): bit k set <=> channel k clamped at 0.  A flag may differ from
+    # the fp64 decision only where the colour itself is within the colour tolerance of 0 on both sides.
+    n_clamp_diff = 0
+    for k in range(3):
+        rb, gb = (ref["clamped"] >> k) & 1, (got["clamped"] >> k) & 1
+        assert not (got["rgb"][vis, k][gb[vis] == 1]).any(), "a channel flagged as clamped must be exactly 0"
+        diff = vis & (rb != gb)
+        n_clamp_diff += int(diff.sum())
+        near0 = np.maximum(np.abs(ref["rgb"][:, k]), np.abs(got["rgb"][:, k])) <= 1e-5
+        assert not (diff & ~near0).any(), f"channel {k}: {(diff & ~near0).sum()} clamp flags differ away from 0"
+    assert not got["clamped"][got["radii"] == 0].any()
     np.testing.assert_allclose(got["depths"], ref["depths"], rtol=2e-6, atol=1e-6)
     np.testing.assert_allclose(got["means2d"][vis], ref["means2d"][vis], rtol=2e-6, atol=5e-4)
     A, B, Cc, o = ref["conic_opacity"][vis].T
@@ -78,7 +88,8 @@ def check_preprocess(fr, sc, cam, max_flag_frac=0.01):
     both = culled & (got["radii"] == 0)
     for k in ("means2d", "conic_opacity", "rgb"):
         assert not got[k][both].any()
-    return dict(n_flagged=int(flag.sum()), n_int_diff=n_flag_diff, n_visible=int(vis.sum()))
+    return dict(n_flagged=int(flag.sum()), n_int_diff=n_flag_diff, n_visible=int(vis.sum()), n_clamp_diff=n_clamp_diff,
+                n_clamped=int(((got["clamped"] > 0) & vis).sum()))
 
 
 def check_bin_sort(fr, cam):

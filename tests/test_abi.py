@@ -68,7 +68,7 @@ def test_invalid_arguments_are_rejected_without_a_gpu(lib):
     rc = lib.mg_bin_sort(C.byref(cam), C.c_int64(-5), *[C.c_void_p(0)] * 3, C.c_uint64(0), C.c_void_p(0), C.c_size_t(0),
                          *[C.c_void_p(0)] * 5)
     assert rc == binding.MG_ERR_INVALID_ARG
-    rc = lib.mg_preprocess(None, C.c_int64(1), *[C.c_void_p(0)] * 15)
+    rc = lib.mg_preprocess(None, C.c_int64(1), *[C.c_void_p(0)] * 16)
     assert rc == binding.MG_ERR_INVALID_ARG
 
 

@@ -31,6 +31,8 @@ def small_scenes():
         # ragged image (partial tiles on both edges), outdoor generator with huge background splats
         "cfg3_small": lambda: scenes.config3(n=60_000, width=333, height=211),
         "cfg4_small": lambda: scenes.config4(n=50_000, width=320, height=208),
+        # long thin splats far from their centres: the terms of the exponent reach 1e4..1e6 and cancel
+        "needles": lambda: scenes.needles(),
     }
 
 
@@ -150,6 +152,62 @@ def test_background_colour(oracle):
     ids, ranges = pu.check_bin_sort(fr, cam)
     pu.check_render_fwd(fr, cam, sc.masks, ids, ranges)
     pu.check_render_bwd(fr, cam, sc.N, sc.masks, ids, ranges, sc.dL_dimage())
+
+
+def test_projection_backward_with_dense_upstream_gradients(oracle):
+    """mg_preprocess_bwd alone at N = 1.2 M with EVERY visible Gaussian carrying a gradient (a view early in training:
+    little saturation).  The geometry kernel queues the Gaussians that need the chain; at this density a block's
+    queue fills several times per sweep.  Compared with the oracle's VJP of the same upstream gradients."""
+    sc = scenes.config3(n=1_200_000, width=640, height=416)
+    cam = sc.camera
+    g, m = mg.upload(sc)
+    fr = mg.Frame(cam, sc.N)
+    fr.preprocess(g)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(5)
+    up = dict(dL_dmeans2d=rng.standard_normal((sc.N, 2)), dL_dconic=rng.standard_normal((sc.N, 3)),
+              dL_dopacity=rng.standard_normal(sc.N), dL_drgb=rng.standard_normal((sc.N, 3)))
+    for k, v in up.items():
+        getattr(fr, k).copy_(torch.from_numpy(v.astype(np.float32)))
+    fr.preprocess_bwd(g)
+    torch.cuda.synchronize()
+    vis = fr.radii.cpu().numpy() > 0
+    assert vis.mean() > 0.5
+    ref5, s5 = pu.check_preprocess_bwd(fr, sc, cam)
+    for k, v in s5.items():
+        assert v <= 2e-4, f"{k}: relative 2-norm error {v:.2e}"
+    # elementwise on a well-conditioned subset: conic -> covariance amplifies the fp32 rounding of the upstream
+    # gradient by the splat's anisotropy squared; random (not rendered) dL/dconic does not cancel the way a real one does
+    for k in ("dL_dopacity_logits", "dL_dsh"):
+        pu.grad_close(pu.f64(getattr(fr, k))[vis], ref5[k][vis], k, rtol=1e-3, floor_frac=1e-4)
+    print("dense upstream", s5)
+
+
+def test_lookback_failure_is_reported_not_returned_as_an_order():
+    """include/mg.h, mg_bin_sort "Internal failure": a look-back that gives up must not yield a wrong order.  Injected
+    through the test hook: every look-back gives up at once."""
+    sc = scenes.config2()
+    g, m = mg.upload(sc)
+    fr = mg.Frame(sc.camera, sc.N)
+    fr.forward(g, m)
+    torch.cuda.synchronize()
+    R = fr.R
+    good = fr.tile_ranges.clone()
+    try:
+        mg.lib().mg_debug_set_lookback_spin_limit(0)
+        fr.sorted_ids.fill_(-1)
+        fr.bin_sort()
+        torch.cuda.synchronize()
+        assert int(fr.R_host[1]) == -1  # UINT64_MAX read as int64
+        assert not fr.tile_ranges.any() and (fr.sorted_ids == -1).all()
+        fr.render_fwd(m)  # harmless: every range is empty
+        torch.cuda.synchronize()
+        assert (fr.n_contrib == 0).all()
+    finally:
+        mg.lib().mg_debug_set_lookback_spin_limit(-1)
+    fr.bin_sort()
+    torch.cuda.synchronize()
+    assert int(fr.R_host[1]) == R and torch.equal(fr.tile_ranges, good)
 
 
 # ------------------------------------------------------------------ edge cases
