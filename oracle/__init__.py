@@ -97,21 +97,28 @@ def bin_sort(cam, depths, rects, tiles_touched, tile_select=None):
     return sorted_ids[:R_out.value], tile_ranges
 
 
+def _counts(out, counts):
+    c = [int(v) for v in counts]
+    out["pair_evals"], out["pair_evals_masked"] = c[0] + c[1], c[1]
+    out["blends"], out["blends_masked"] = c[2] + c[3], c[3]
+
+
 def render_fwd(cam, sorted_ids, tile_ranges, means2d, conic_opacity, rgb, masks):
-    """O10.  Returns dict(image [3,H,W], final_T, n_contrib, margin, hash, pair_evals, blends)."""
+    """O10.  Returns dict(image [3,H,W], final_T, n_contrib, margin, hash) + the work counters of SURVEY.md 8(d):
+    pair_evals / blends (totals) and pair_evals_masked / blends_masked (the part on entries with M == 0)."""
     H, W = cam.height, cam.width
     sorted_ids, tile_ranges = _in(sorted_ids, np.uint32), _in(tile_ranges, np.uint32)
     means2d, conic_opacity, rgb = _in(means2d, np.float64), _in(conic_opacity, np.float64), _in(rgb, np.float64)
     masks = _in(masks, np.float32)
     out = dict(image=np.zeros((3, H, W)), final_T=np.zeros((H, W)), n_contrib=np.zeros((H, W), np.uint32),
                margin=np.zeros((H, W)), hash=np.zeros((H, W), np.uint64))
-    counts = np.zeros(2, np.uint64)
+    counts = np.zeros(4, np.uint64)
     c = _cam(cam)
     rc = lib().orc_render_fwd(C.byref(c), _p(sorted_ids), _p(tile_ranges), _p(means2d), _p(conic_opacity), _p(rgb),
                               _p(masks), _p(out["image"]), _p(out["final_T"]), _p(out["n_contrib"]), _p(out["margin"]),
                               _p(out["hash"]), _p(counts))
     assert rc == 0
-    out["pair_evals"], out["blends"] = int(counts[0]), int(counts[1])
+    _counts(out, counts)
     return out
 
 
@@ -123,14 +130,14 @@ def render_bwd(cam, N, sorted_ids, tile_ranges, means2d, conic_opacity, rgb, mas
     assert dL_dimage.shape == (3, cam.height, cam.width)
     out = dict(dL_dmeans2d=np.zeros((N, 2)), dL_dconic=np.zeros((N, 3)), dL_dopacity=np.zeros(N),
                dL_drgb=np.zeros((N, 3)), dL_dmask=np.zeros(N), sens=np.zeros(N, np.uint32))
-    counts = np.zeros(2, np.uint64)
+    counts = np.zeros(4, np.uint64)
     c = _cam(cam)
     rc = lib().orc_render_bwd(C.byref(c), C.c_int64(N), _p(sorted_ids), _p(tile_ranges), _p(means2d), _p(conic_opacity),
                               _p(rgb), _p(masks), _p(dL_dimage), _p(out["dL_dmeans2d"]), _p(out["dL_dconic"]),
                               _p(out["dL_dopacity"]), _p(out["dL_drgb"]), _p(out["dL_dmask"]),
                               _p(out["sens"]) if cutoff > 0 else None, C.c_double(cutoff), _p(counts))
     assert rc == 0
-    out["pair_evals"], out["blends"] = int(counts[0]), int(counts[1])
+    _counts(out, counts)
     return out
 
 

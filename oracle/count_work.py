@@ -4,7 +4,11 @@
 
 A pair evaluation = one (list entry, pixel) visited before the pixel stops; a blend = a pair evaluation
 that passes the alpha filter, masked or not.  Backward counts are the pairs the reverse
-traversal revisits (positions last..1) and the blends among them.  Camera 0 of each config.
+traversal revisits (positions n_contrib..1) and the blends among them.  Every count also comes split by the
+entry's mask (`*_masked` = the part on entries with M == 0): under DESIGN.md reading 5 the forward pass never
+has to look at a masked entry and the backward pass owes it dL/dM only, so the algorithmic flop counts of
+bench.py charge the two kinds differently.  Camera 0 of each config.  The counters are pinned by
+tests/test_oracle_pins.py::test_work_counters_match_an_independent_count.
 """
 import json
 import os
@@ -30,7 +34,9 @@ def count(cfg: int) -> dict:
     lens = (ranges[:, 1] - ranges[:, 0]).astype(np.int64)
     return dict(config=cfg, N=sc.N, width=cam.width, height=cam.height, visible=int((pre["radii"] > 0).sum()),
                 R=int(len(ids)), fwd_pair_evals=fwd["pair_evals"], fwd_blends=fwd["blends"],
+                fwd_pair_evals_masked=fwd["pair_evals_masked"], fwd_blends_masked=fwd["blends_masked"],
                 bwd_pair_evals=rb["pair_evals"], bwd_blends=rb["blends"],
+                bwd_pair_evals_masked=rb["pair_evals_masked"], bwd_blends_masked=rb["blends_masked"],
                 stopped_pixels=int((fwd["final_T"] < 1e-3).sum()), list_len_max=int(lens.max()),
                 list_len_median=int(np.median(lens)), oracle_seconds=round(time.time() - t, 1))
 

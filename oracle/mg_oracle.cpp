@@ -310,16 +310,21 @@ int orc_bin_sort(const Cam* cam, int64_t N, const float* depths, const int32_t* 
 // nothing stopped it (reading 5).  Every entry the reverse traversal must visit lies at a
 // position <= last, and no entry at or behind the stop does.  `margin` receives the smallest
 // relative distance of any decision from its flip point; `hash` a signature of all decisions.
+// Work counters ("a pair evaluation = one (list entry, pixel) visited before the pixel stops; a
+// blend = a pair evaluation that passes the alpha filter, masked or not"), split by the entry's mask:
+//   cnt[0] / cnt[1]: entries visited with M != 0 / M == 0 (the entry that stops the pixel is visited: cnt[0]);
+//   cnt[2] / cnt[3]: those of them that pass the alpha filter (the stopping entry passes it: cnt[2]).
 static double walk_pixel(double px, double py, const uint32_t* ids, uint32_t n, const double* means2d,
                          const double* conic_opacity, const float* masks, std::vector<Passing>* pass, uint32_t* last,
-                         double* margin, double* margin_clamp, uint64_t* hash, uint64_t* n_eval, uint64_t* n_blend) {
+                         double* margin, double* margin_clamp, uint64_t* hash, uint64_t* cnt) {
   double T = 1.0, mg = 1e30, mgc = 1e30;
   uint64_t h = 1469598103934665603ull;
   auto mix = [&](uint64_t v) { h = (h ^ v) * 1099511628211ull; };
   *last = n;
   for (uint32_t k = 0; k < n; k++) {
     const uint32_t id = ids[k];
-    (*n_eval)++;
+    const int masked = masks[id] == 0.0f ? 1 : 0;
+    cnt[masked]++;
     const double dx = means2d[2 * (int64_t)id] - px, dy = means2d[2 * (int64_t)id + 1] - py;
     const double* co = conic_opacity + 4 * (int64_t)id;
     const double power = -0.5 * (co[0] * dx * dx + 2.0 * co[1] * dx * dy + co[2] * dy * dy);
@@ -329,7 +334,7 @@ static double walk_pixel(double px, double py, const uint32_t* ids, uint32_t n, 
     const double alpha = std::min(ALPHA_MAX, oG);
     mg = std::min(mg, std::fabs(alpha - ALPHA_MIN) / ALPHA_MIN);
     if (alpha < ALPHA_MIN) { mix(id * 4ull + 1); continue; }  // the mask is NOT consulted
-    (*n_blend)++;
+    cnt[2 + masked]++;
     mgc = std::min(mgc, std::fabs(oG - ALPHA_MAX) / ALPHA_MAX);
     const double a = (double)masks[id] * alpha;  // Eq. 4: T_{i+1} = (1 - M_i alpha_i) T_i
     const double Tn = T * (1.0 - a);
@@ -347,14 +352,15 @@ static double walk_pixel(double px, double py, const uint32_t* ids, uint32_t n, 
 
 // O10 forward: image = sum M_i c_i alpha_i T_i (Eq. 3) + T_{N+1} bg (Eq. 9-10).
 // image [3][H][W], final_T [H][W], n_contrib [H][W] (number of list entries consumed before the stop,
-// reading 5), margin [H][W], hash [H][W], counts[2] = {pair evaluations, blends}.
+// reading 5), margin [H][W], hash [H][W], counts[4] = walk_pixel's work counters summed over the pixels
+// {pair evaluations M != 0, M == 0, blends M != 0, M == 0}.
 int orc_render_fwd(const Cam* cam, const uint32_t* sorted_ids, const uint32_t* tile_ranges, const double* means2d,
                    const double* conic_opacity, const double* rgb, const float* masks, double* image, double* final_T,
                    uint32_t* n_contrib, double* margin, uint64_t* hash, uint64_t* counts) {
   const int W = cam->width, H = cam->height;
   const int gw = (W + TILE - 1) / TILE, gh = (H + TILE - 1) / TILE;
-  uint64_t tot_eval = 0, tot_blend = 0;
-#pragma omp parallel for schedule(dynamic, 1) reduction(+ : tot_eval, tot_blend)
+  uint64_t tot0 = 0, tot1 = 0, tot2 = 0, tot3 = 0;
+#pragma omp parallel for schedule(dynamic, 1) reduction(+ : tot0, tot1, tot2, tot3)
   for (int t = 0; t < gw * gh; t++) {
     const uint32_t s = tile_ranges[2 * t], e = tile_ranges[2 * t + 1];
     std::vector<Passing> pass;
@@ -363,8 +369,8 @@ int orc_render_fwd(const Cam* cam, const uint32_t* sorted_ids, const uint32_t* t
         pass.clear();
         uint32_t last;
         double mg, mgc;
-        uint64_t h, ne = 0, nb = 0;
-        const double T = walk_pixel(px, py, sorted_ids + s, e - s, means2d, conic_opacity, masks, &pass, &last, &mg, &mgc, &h, &ne, &nb);
+        uint64_t h, cnt[4] = {0, 0, 0, 0};
+        const double T = walk_pixel(px, py, sorted_ids + s, e - s, means2d, conic_opacity, masks, &pass, &last, &mg, &mgc, &h, cnt);
         double C[3] = {0, 0, 0};
         for (const Passing& p : pass)
           for (int k = 0; k < 3; k++) C[k] += p.a * p.T * rgb[3 * (int64_t)p.id + k];
@@ -374,11 +380,10 @@ int orc_render_fwd(const Cam* cam, const uint32_t* sorted_ids, const uint32_t* t
         n_contrib[pix] = last;
         if (margin) margin[pix] = mg;
         if (hash) hash[pix] = h;
-        tot_eval += ne;
-        tot_blend += nb;
+        tot0 += cnt[0]; tot1 += cnt[1]; tot2 += cnt[2]; tot3 += cnt[3];
       }
   }
-  if (counts) { counts[0] = tot_eval; counts[1] = tot_blend; }
+  if (counts) { counts[0] = tot0; counts[1] = tot1; counts[2] = tot2; counts[3] = tot3; }
   return 0;
 }
 
@@ -386,7 +391,9 @@ int orc_render_fwd(const Cam* cam, const uint32_t* sorted_ids, const uint32_t* t
 // Eq. 11 from the back, then Eq. 18 for dL/dM_i; dL/dalpha_i = M_i * (same bracket); colour and
 // alpha chain to (mean2d, conic, opacity).  All sums in fp64.
 // sens[N] (optional): +1 for every pixel with a decision margin below `cutoff` at which the
-// Gaussian was visited with alpha >= (1-cutoff)/255.  counts[2] = {pair evals, blends} revisited.
+// Gaussian was visited with alpha >= (1-cutoff)/255.  counts[4] = the work of the reverse traversal, which revisits
+// positions n_contrib..1 of every pixel: {pair evaluations M != 0, M == 0, blends M != 0, M == 0} (the entry
+// that stopped the pixel lies behind n_contrib and is not revisited).
 int orc_render_bwd(const Cam* cam, int64_t N, const uint32_t* sorted_ids, const uint32_t* tile_ranges,
                    const double* means2d, const double* conic_opacity, const double* rgb, const float* masks,
                    const double* dL_dimage, double* dL_dmeans2d, double* dL_dconic, double* dL_dopacity,
@@ -401,8 +408,8 @@ int orc_render_bwd(const Cam* cam, int64_t N, const uint32_t* sorted_ids, const 
     dL_dmask[i] = 0;
     if (sens) sens[i] = 0;
   }
-  uint64_t tot_eval = 0, tot_blend = 0;
-#pragma omp parallel for schedule(dynamic, 1) reduction(+ : tot_eval, tot_blend)
+  uint64_t tot0 = 0, tot1 = 0, tot2 = 0, tot3 = 0;
+#pragma omp parallel for schedule(dynamic, 1) reduction(+ : tot0, tot1, tot2, tot3)
   for (int t = 0; t < gw * gh; t++) {
     const uint32_t s = tile_ranges[2 * t], e = tile_ranges[2 * t + 1];
     const uint32_t n = e - s;
@@ -415,14 +422,19 @@ int orc_render_bwd(const Cam* cam, int64_t N, const uint32_t* sorted_ids, const 
         pass.clear();
         uint32_t last;
         double mg, mgc;
-        uint64_t h, ne = 0, nb = 0;
-        const double Tfin = walk_pixel(px, py, sorted_ids + s, n, means2d, conic_opacity, masks, &pass, &last, &mg, &mgc, &h, &ne, &nb);
+        uint64_t h, cnt[4] = {0, 0, 0, 0};
+        const double Tfin = walk_pixel(px, py, sorted_ids + s, n, means2d, conic_opacity, masks, &pass, &last, &mg, &mgc, &h, cnt);
+        const uint64_t ne = cnt[0] + cnt[1];  // entries the forward walk visited (incl. the stopping one)
         const int64_t pix = (int64_t)py * W + px;
         const double g[3] = {dL_dimage[pix], dL_dimage[(int64_t)H * W + pix], dL_dimage[(int64_t)2 * H * W + pix]};
         const double gbg = g[0] * cam->bg[0] + g[1] * cam->bg[1] + g[2] * cam->bg[2];
         double Bc[3] = {0, 0, 0};  // b_{i+1}: colour rendered behind the current entry (Eq. 11), b_{N+1} = 0
-        tot_eval += last;           // the reverse traversal revisits positions last..1
-        tot_blend += pass.size();
+        for (uint32_t k = 0; k < last; k++) {  // the reverse traversal revisits positions last..1
+          if (masks[sorted_ids[s + k]] == 0.0f) tot1++; else tot0++;
+        }
+        for (const Passing& p : pass) {
+          if (masks[p.id] == 0.0f) tot3++; else tot2++;
+        }
         for (size_t kk = pass.size(); kk-- > 0;) {
           const Passing& p = pass[kk];
           const double* c = rgb + 3 * (int64_t)p.id;
@@ -490,7 +502,7 @@ int orc_render_bwd(const Cam* cam, int64_t N, const uint32_t* sorted_ids, const 
       }
     }
   }
-  if (counts) { counts[0] = tot_eval; counts[1] = tot_blend; }
+  if (counts) { counts[0] = tot0; counts[1] = tot1; counts[2] = tot2; counts[3] = tot3; }
   return 0;
 }
 

@@ -29,7 +29,7 @@ def test_full_size_projection_and_sort(full, oracle):
     s1 = pu.check_preprocess(fr, sc, cam, max_flag_frac=0.02)
     ids, ranges = pu.check_bin_sort(fr, cam)
     assert fr.R > 10_000_000
-    print(sc.name, "preprocess", s1, "R", fr.R)
+    print("PARITY", sc.name, "full size", dict(R=fr.R, preprocess=s1))
 
 
 def test_full_size_blend_on_sampled_tiles(full, oracle):
@@ -46,7 +46,7 @@ def test_full_size_blend_on_sampled_tiles(full, oracle):
     ranges_s[tiles] = ranges_full[tiles]
     ids = pu.u32(fr.sorted_ids)[: fr.R]
     ref, s3 = pu.check_render_fwd(fr, cam, sc.masks, ids, ranges_s, tiles=tiles, max_flag_frac=0.05)
-    print(sc.name, "fwd sampled tiles", len(tiles), s3)
+    print("PARITY", sc.name, "full size fwd sampled tiles", dict(tiles=len(tiles), render_fwd=s3))
     # backward restricted to the same tiles on both sides
     keep_ranges = fr.tile_ranges.clone()
     fr.tile_ranges.copy_(torch.from_numpy(ranges_s.view(np.int32)).cuda())
@@ -54,11 +54,45 @@ def test_full_size_blend_on_sampled_tiles(full, oracle):
     torch.cuda.synchronize()
     try:
         _, s4 = pu.check_render_bwd(fr, cam, sc.N, sc.masks, ids, ranges_s, sc.dL_dimage(), max_flag_frac=0.3)
-        print(sc.name, "bwd sampled tiles", {k: round(v, 4) for k, v in s4.items()})
+        print("PARITY", sc.name, "full size bwd sampled tiles", dict(render_bwd=s4))
     finally:
         fr.tile_ranges.copy_(keep_ranges)
         fr.render_bwd(m, gimg)
         torch.cuda.synchronize()
+
+
+@pytest.mark.parametrize("cam_index", [5, 10, 15])
+def test_config5_other_cameras_on_the_circle(oracle, cam_index):
+    """BASELINE.json configs[4]: "timed over 20 cameras on a circle of radius 8".  Camera 0 is the `full` fixture; the
+    same full-size checks for three more of the 20 views (the scene looks different from every side: other Gaussians
+    are culled, other depth order, other R): projection on all 6 M Gaussians, the sort on all keys bit-exactly, both
+    blend kernels on sampled tiles, projection backward in the 2-norm."""
+    sc = scenes.make(5)
+    cam = sc.cameras[cam_index]
+    fr, g, m, gimg = pu.run_gpu(sc, cam_index=cam_index)
+    s1 = pu.check_preprocess(fr, sc, cam, max_flag_frac=0.02)
+    ids, ranges = pu.check_bin_sort(fr, cam)
+    assert fr.R > 40_000_000
+    gw, gh = mg.grid(cam)
+    lens = (ranges[:, 1].astype(np.int64) - ranges[:, 0])
+    tiles = sorted(set(np.random.default_rng(cam_index).choice(gw * gh, 20, replace=False).tolist()) | {int(np.argmax(lens)), gw * gh - 1})
+    ranges_s = np.zeros_like(ranges)
+    ranges_s[tiles] = ranges[tiles]
+    _, s3 = pu.check_render_fwd(fr, cam, sc.masks, ids, ranges_s, tiles=tiles, max_flag_frac=5e-3)
+    fr.tile_ranges.copy_(torch.from_numpy(ranges_s.view(np.int32)).cuda())
+    fr.render_bwd(m, gimg)
+    torch.cuda.synchronize()
+    _, s4 = pu.check_render_bwd(fr, cam, sc.N, sc.masks, ids, ranges_s, sc.dL_dimage(cam_index), max_flag_frac=2e-3)
+    fr.tile_ranges.copy_(torch.from_numpy(ranges.view(np.int32)).cuda())
+    fr.render_bwd(m, gimg)
+    fr.preprocess_bwd(g)
+    torch.cuda.synchronize()
+    _, s5 = pu.check_preprocess_bwd(fr, sc, cam)
+    for k, v in s5.items():
+        assert v <= 2e-4, f"{k}: relative 2-norm error {v:.2e}"
+    print("PARITY", f"cfg5 camera {cam_index}", dict(R=fr.R, preprocess=s1, render_fwd=s3, render_bwd=s4, preprocess_bwd=s5))
+    del fr, g, m, gimg
+    torch.cuda.empty_cache()
 
 
 def test_full_size_projection_backward(full, oracle):
@@ -67,7 +101,7 @@ def test_full_size_projection_backward(full, oracle):
     ref5, s5 = pu.check_preprocess_bwd(fr, sc, cam)
     for k, v in s5.items():
         assert v <= 2e-4, f"{k}: relative 2-norm error {v:.2e}"
-    print(sc.name, "preprocess_bwd", s5)
+    print("PARITY", sc.name, "full size", dict(preprocess_bwd=s5))
 
 
 def test_full_size_invariants(full):

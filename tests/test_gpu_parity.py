@@ -23,6 +23,11 @@ def _need_gpu():
     mg.lib()  # fails loudly if libmg.so is missing: there is no fallback
 
 
+# Largest fraction of Gaussians the end-to-end gradient comparison may exempt as threshold-sensitive (about twice the
+# count observed on the B200, profiles/r02_parity_counts.md).
+E2E_GRAD_BUDGET = {"tiny": 0.0, "cfg1": 0.2, "cfg2": 0.5, "cfg3_small": 0.2, "cfg4_small": 0.2, "needles": 0.5}
+
+
 def small_scenes():
     return {
         "tiny": lambda: scenes.tiny_fd_scene(),
@@ -56,7 +61,7 @@ def test_staged_parity_all_five_calls(run, oracle):
         assert v <= 1e-4, f"{k}: relative 2-norm error {v:.2e}"
     for k in ref5:
         pu.grad_close(pu.f64(getattr(fr, k))[vis], ref5[k][vis], k, rtol=1e-3, floor_frac=1e-4)
-    print(name, s1, s3, {k: round(v, 4) for k, v in s4.items()}, s5)
+    print("PARITY", name, "staged", dict(preprocess=s1, render_fwd=s3, render_bwd=s4, preprocess_bwd=s5))
 
 
 def test_end_to_end_image_parity(run, oracle):
@@ -85,17 +90,30 @@ def test_end_to_end_image_parity(run, oracle):
 
 
 def test_end_to_end_gradient_parity(run, oracle):
+    """fp64 oracle from the raw inputs vs the GPU's gradients w.r.t. the raw inputs and the masks: ELEMENTWISE (1e-3
+    relative) on every Gaussian the oracle does not flag as threshold-sensitive at CUT_E2E and whose integer decisions
+    (radius, rect) agree between fp32 and fp64, plus the 2-norm over all of them."""
     name, sc, fr = run
     cam = sc.camera
     g = sc.dL_dimage().astype(np.float64)
     pre, ids, ranges, fwd = oracle.full_forward(cam, pu.arrays(sc), sc.masks)
-    rb, pb = oracle.full_backward(cam, pu.arrays(sc), sc.masks, pre, ids, ranges, g)
-    for k, ref in list(rb.items()) + list(pb.items()):
-        if not k.startswith("dL_"):
-            continue
-        got = pu.f64(getattr(fr, k))
-        rel = np.linalg.norm(got - ref) / max(np.linalg.norm(ref), 1e-300)
-        assert rel < 2e-3, f"{name} {k}: relative 2-norm error {rel:.2e}"
+    rb, pb = oracle.full_backward(cam, pu.arrays(sc), sc.masks, pre, ids, ranges, g, cutoff=pu.CUT_E2E)
+    gpu = pu.gpu_pre(fr)
+    unstable = (pre["radii"] != gpu["radii"]) | (pre["rects"] != gpu["rects"]).any(1)
+    # a Gaussian whose rect differs changes the lists of the tiles at its border: the pixels there (and the Gaussians
+    # blended behind it at those pixels) see one entry more or less.  Scenes with such Gaussians are compared in the
+    # 2-norm only; the others elementwise on the non-flagged Gaussians.
+    order_same = fr.R == len(ids) and np.array_equal(pu.u32(fr.sorted_ids)[: fr.R], ids)
+    clean = (rb["sens"] == 0) & ~unstable
+    ref = {k: v for k, v in list(rb.items()) + list(pb.items()) if k.startswith("dL_")}
+    if order_same:
+        out = pu.grads_vs_ref(fr, ref, list(ref), clean, max_flag_frac=E2E_GRAD_BUDGET[name], l2_clean=2e-4)
+    else:
+        out = {}
+        for k, r in ref.items():
+            out[k + "_l2"] = float(np.linalg.norm(pu.f64(getattr(fr, k)) - r) / max(np.linalg.norm(r), 1e-300))
+            assert out[k + "_l2"] < pu.L2_ALL, f"{name} {k}: relative 2-norm error {out[k + '_l2']:.2e}"
+    print("PARITY", name, "e2e gradients", dict(order_same=bool(order_same), unstable=int(unstable.sum()), **out))
 
 
 def test_masked_gaussians_get_only_mask_gradient(run):

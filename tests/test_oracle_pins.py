@@ -546,3 +546,133 @@ def test_fd_render_stage_gradients(oracle):
                 an = rb[gname].reshape(-1)[k]
             assert abs(fd - an) <= 2e-6 * max(1.0, abs(an)) + 1e-7, (key, k, fd, an)
     assert n_ok > 50
+
+
+# ---------------------------------------------------------------- work counters (numerators of bench.py's throughput)
+def np_pixel_margins(px, py, ids, m2, co, m):
+    """Decision margins of one pixel, from DESIGN.md section 5's definition ("the smallest relative distance of any
+    decision the walk took from its flip point"), written with numpy array operations on the whole list."""
+    if len(ids) == 0:
+        return np.inf, np.inf, 0, np.zeros(0)
+    d = m2[ids] - np.array([px, py], float)
+    A, B, C, o = co[ids].T
+    power = -0.5 * (A * d[:, 0] ** 2 + 2 * B * d[:, 0] * d[:, 1] + C * d[:, 1] ** 2)
+    oG = o * np.exp(np.minimum(power, 0.0))
+    alpha = np.minimum(ALPHA_MAX, oG)
+    ok = (power <= 0) & (alpha >= ALPHA_MIN)
+    a = np.where(ok, m[ids] * alpha, 0.0)
+    Tn = np.cumprod(1 - a)
+    stop = np.nonzero(ok & (Tn < T_MIN))[0]
+    nvis = stop[0] + 1 if len(stop) else len(ids)  # entries visited, the stopping one included
+    v = slice(0, nvis)
+    inside = power[v] <= 0
+    mg_alpha = (np.abs(alpha[v] - ALPHA_MIN) / ALPHA_MIN)[inside]
+    mg_T = (np.abs(Tn[v] - T_MIN) / T_MIN)[ok[v]]
+    mg_clamp = (np.abs(oG[v] - ALPHA_MAX) / ALPHA_MAX)[ok[v]]
+    mg = min(mg_alpha.min() if mg_alpha.size else np.inf, mg_T.min() if mg_T.size else np.inf)
+    return mg, (mg_clamp.min() if mg_clamp.size else np.inf), nvis, alpha[v]
+
+
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_work_counters_match_an_independent_count(oracle, cfg):
+    """"a pair evaluation = one (list entry, pixel) visited before the pixel stops; a blend = a pair
+    evaluation that passes the alpha filter (masked or not)".  The oracle's counters (numerators of every throughput
+    and roofline number of bench.py) against a count taken from the numpy Eq. 3-4 loop, masked and unmasked entries
+    separately, forward (the stopping entry is visited and passes the filter) and backward (positions n_contrib..1)."""
+    sc = scenes.config1() if cfg == 1 else scenes.config2(n=60000, width=128, height=96)  # cfg 2: ~800 pixels stop
+    cam = sc.camera
+    pre, ids, ranges, fwd = oracle.full_forward(cam, arrays(sc), sc.masks)
+    g = sc.dL_dimage().astype(np.float64)
+    rb = oracle.render_bwd(cam, sc.N, ids, ranges, pre["means2d"], pre["conic_opacity"], pre["rgb"], sc.masks, g)
+    gw = (cam.width + 15) // 16
+    f_ev = [0, 0]; f_bl = [0, 0]; b_ev = [0, 0]; b_bl = [0, 0]  # [unmasked, masked]
+    n_stopped = 0
+    for py in range(cam.height):
+        for px in range(cam.width):
+            s, e = ranges[(py // 16) * gw + px // 16]
+            lst = ids[s:e]
+            _, _, n, _, _, ok = np_pixel(px, py, lst, pre["means2d"], pre["conic_opacity"], pre["rgb"], sc.masks, cam.bg)
+            stopped = n < len(lst)
+            n_stopped += stopped
+            mk = sc.masks[lst[:n]] == 0
+            for j, sel in enumerate((~mk, mk)):
+                b_ev[j] += int(sel.sum()); b_bl[j] += int((ok & sel).sum())
+                f_ev[j] += int(sel.sum()); f_bl[j] += int((ok & sel).sum())
+            if stopped:  # the entry that stops the pixel: visited, passes the filter, never masked (reading 3)
+                assert sc.masks[lst[n]] != 0
+                f_ev[0] += 1; f_bl[0] += 1
+    assert (fwd["pair_evals"] - fwd["pair_evals_masked"], fwd["pair_evals_masked"]) == tuple(f_ev)
+    assert (fwd["blends"] - fwd["blends_masked"], fwd["blends_masked"]) == tuple(f_bl)
+    assert (rb["pair_evals"] - rb["pair_evals_masked"], rb["pair_evals_masked"]) == tuple(b_ev)
+    assert (rb["blends"] - rb["blends_masked"], rb["blends_masked"]) == tuple(b_bl)
+    assert fwd["pair_evals"] - rb["pair_evals"] == n_stopped == fwd["blends"] - rb["blends"]
+    assert f_ev[1] > 0 and f_bl[1] > 0 and (cfg == 1 or n_stopped > 0)
+    # the committed table the bench reads was written from these counters
+    import json, os
+    wc = json.load(open(os.path.join(os.path.dirname(__file__), "..", "oracle", "work_counts.json")))
+    if cfg == 1:
+        assert wc["1"]["fwd_pair_evals"] == fwd["pair_evals"] and wc["1"]["bwd_blends_masked"] == rb["blends_masked"]
+
+
+def test_bin_sort_tile_select_is_the_full_result_restricted_to_the_selected_tiles(oracle):
+    """orc_bin_sort's tile_select branch (bench.py's bounded cpu_baseline sample): selected tiles keep exactly the
+    list of the unselected run, the others are empty, R = the sum of the kept lists."""
+    sc = scenes.config2(n=20000, width=256, height=256)
+    cam = sc.camera
+    pre = oracle.preprocess(cam, *arrays(sc))
+    d32 = pre["depths"].astype(np.float32)
+    ids, ranges = oracle.bin_sort(cam, d32, pre["rects"], pre["tiles_touched"])
+    ntiles = ranges.shape[0]
+    sel = np.zeros(ntiles, np.uint8)
+    sel[1::3] = 1
+    ids_s, ranges_s = oracle.bin_sort(cam, d32, pre["rects"], pre["tiles_touched"], sel)
+    kept = 0
+    for t in range(ntiles):
+        s, e = ranges_s[t]
+        if sel[t]:
+            assert np.array_equal(ids_s[s:e], ids[ranges[t, 0]:ranges[t, 1]])
+            kept += int(e - s)
+        else:
+            assert s == e
+    assert kept == len(ids_s) and 0 < kept < len(ids)
+    assert (np.diff(ranges_s.reshape(-1).astype(np.int64)) >= 0).all()  # ranges tile the array in tile order
+
+
+def test_margins_and_sens_flags_follow_their_definition(oracle, cfg1):
+    """The per-pixel decision margin and the per-Gaussian `sens` count decide which elements a GPU parity test may
+    exempt.  (a) Both against a numpy evaluation of DESIGN.md section 5's definition.  (b) The property they exist
+    for: perturbing the render-stage inputs by fp32-sized relative amounts changes decisions only at pixels whose
+    margin is below the cut-off, and moves the gradient only of Gaussians with sens > 0 beyond the tolerance."""
+    sc, pre, ids, ranges, fwd = cfg1
+    cam = sc.camera
+    gw = (cam.width + 15) // 16
+    cut = 2e-4
+    g = sc.dL_dimage().astype(np.float64)
+    rb = oracle.render_bwd(cam, sc.N, ids, ranges, pre["means2d"], pre["conic_opacity"], pre["rgb"], sc.masks, g, cutoff=cut)
+    sens = np.zeros(sc.N, np.int64)
+    for py in range(cam.height):
+        for px in range(cam.width):
+            s, e = ranges[(py // 16) * gw + px // 16]
+            lst = ids[s:e]
+            mg, mgc, nvis, alpha = np_pixel_margins(px, py, lst, pre["means2d"], pre["conic_opacity"], sc.masks)
+            if np.isfinite(mg):
+                np.testing.assert_allclose(fwd["margin"][py, px], mg, rtol=1e-9)
+            else:
+                assert fwd["margin"][py, px] > 1e29
+            if min(mg, mgc) < cut:
+                np.add.at(sens, lst[:nvis][alpha >= (1 - cut) * ALPHA_MIN], 1)
+    assert np.array_equal(sens, rb["sens"].astype(np.int64)) and sens.sum() > 0
+    # (b) relative perturbation of 2e-7 (a few fp32 ulps) of centres, conics and opacities
+    rng = np.random.default_rng(9)
+    m2p = pre["means2d"] * (1 + 2e-7 * rng.uniform(-1, 1, pre["means2d"].shape))
+    cop = pre["conic_opacity"] * (1 + 2e-7 * rng.uniform(-1, 1, pre["conic_opacity"].shape))
+    fwd_p = oracle.render_fwd(cam, ids, ranges, m2p, cop, pre["rgb"], sc.masks)
+    changed = fwd_p["hash"] != fwd["hash"]
+    assert not (changed & (fwd["margin"] >= cut)).any()
+    rb_p = oracle.render_bwd(cam, sc.N, ids, ranges, m2p, cop, pre["rgb"], sc.masks, g)
+    for k in ("dL_dmask", "dL_dopacity", "dL_drgb"):
+        ref = rb[k]
+        err = np.abs(rb_p[k] - ref)
+        tol = 1e-3 * np.abs(ref) + 1e-5 * np.abs(ref).max()
+        bad = (err > tol).reshape(sc.N, -1).any(1)
+        assert not (bad & (rb["sens"] == 0)).any(), k
