@@ -2,12 +2,14 @@
 // Eq. 3-4: C += M_i alpha_i T_i c_i,  T_{i+1} = (1 - M_i alpha_i) T_i;
 // Eq. 9-10: image = C + T_{N+1} c_bg.  Thresholds: DESIGN.md readings 1-5.
 //
-// FP32-pipe bound (no dense contraction on this path, so no tensor cores).  Design (render_common.cuh):
+// FP32-issue bound (no dense contraction on this path, so no tensor cores).  Design (render_common.cuh):
 //  * 2 independent warps per tile, each a 16x8 strip of four 8x4 sub-blocks, one pixel of each per lane;
-//  * per warp, 32 list entries at a time: attributes gathered one batch ahead (cp.async), a 4-bit sub-block reach
-//    mask per entry (lanes = entries), a ballot, then the surviving entries in list order;
-//  * per surviving entry only the reachable, still-live sub-blocks are evaluated; the alpha filter is two
-//    compares on the exponent, the exponential is taken only for pairs that pass;
+//  * per warp, 32 list entries at a time: attributes gathered one batch ahead (cp.async), the record of the entry
+//    expanded about the strip's centre and a 4-bit sub-block reach mask per entry (lanes = entries), a ballot, then the
+//    surviving entries in list order;
+//  * per surviving entry only the reachable, still-live pairs of sub-blocks are evaluated, two pixels per packed
+//    FP32 instruction; the alpha filter is two compares on the exponent, the exponential is taken only for pixels
+//    that pass;
 //  * an entry with M = 0 changes neither C nor T and cannot stop a pixel, and n_contrib counts
 //    the entries consumed before the stop (include/mg.h, reading 5), so masked entries are dropped when the
 //    batch is staged: the forward pass costs nothing for them;
@@ -36,25 +38,28 @@ __global__ void __launch_bounds__(RN_THREADS, RN_FWD_MINB) render_fwd_kernel(
   const int n = (int)(range.y - range.x);
   const uint32_t* ids = sorted_ids + range.x;
 
-  // pixels of this lane: (px[bx], py[by]), sub-block k = 2*by + bx
+  // pixels of this lane: (px[c], py[r]); sub-block k = c + 2 r; pair c = the sub-blocks k = c and k = c + 2
   const int X0i = tx * MG_TILE, Y0i = ty * MG_TILE + 8 * warp;
   const int px[2] = {X0i + (lane & 7), X0i + 8 + (lane & 7)};
   const int py[2] = {Y0i + (lane >> 3), Y0i + 4 + (lane >> 3)};
-  const float fx[2] = {(float)px[0], (float)px[1]}, fy[2] = {(float)py[0], (float)py[1]};
-  const float X0 = (float)X0i, Y0 = (float)Y0i;
+  const float Xc = (float)X0i + 7.5f, Yc = (float)Y0i + 3.5f;  // centre of the strip: origin of the records
+  const RnLane L = rn_lane(lane);
 
-  float T[4], Cr[4], Cg[4], Cb[4];
+  float2 T[2], Cr[2], Cg[2], Cb[2];  // [c], packed over r
+  // [k]: entries consumed = the whole list unless a stop says less.  A pixel is still running at list position pos
+  // iff pos <= last[k]; pixels outside the image never run (0).
   uint32_t last[4];
-  uint32_t live = 0;  // bit k set = pixel k still running.  Pixels outside the image never run.
 #pragma unroll
-  for (int k = 0; k < 4; k++) {
-    T[k] = 1.f; Cr[k] = Cg[k] = Cb[k] = 0.f; last[k] = (uint32_t)n;  // entries consumed unless a stop says less
-    if (px[k & 1] < W && py[k >> 1] < H) live |= 1u << k;
+  for (int c = 0; c < 2; c++) {
+    T[c] = make_float2(1.f, 1.f);
+    Cr[c] = Cg[c] = Cb[c] = make_float2(0.f, 0.f);
   }
+#pragma unroll
+  for (int k = 0; k < 4; k++) last[k] = (px[k & 1] < W && py[k >> 1] < H) ? (uint32_t)n : 0u;
   uint32_t live_sb = 0;  // warp-uniform: bit k set = sub-block k has a running pixel
 #pragma unroll
   for (int k = 0; k < 4; k++)
-    if (__any_sync(0xffffffffu, (live >> k) & 1u)) live_sb |= 1u << k;
+    if (__any_sync(0xffffffffu, last[k] != 0u)) live_sb |= 1u << k;
 
   if (n > 0 && live_sb) {
     // prologue: gather of batch 0 in flight, ids of batch 1 in a register
@@ -67,11 +72,14 @@ __global__ void __launch_bounds__(RN_THREADS, RN_FWD_MINB) render_fwd_kernel(
       __syncwarp();            // every lane is done reading the previous batch's records
       uint32_t m4 = 0;
       if (base + lane < n) {
-        RnRecord rec = rn_make_record(rn_stage_read(stage, lane));
+        const RnRaw raw = rn_stage_read(stage, lane);
         // an entry with M = 0 changes neither C nor T and cannot stop a pixel: dropped here
-        if (rec.b.z != 0.f) m4 = rn_subblock_mask(rec.a, rec.b, X0, Y0) & live_sb;
-        rec.c.w = __uint_as_float(m4);
-        buf[lane] = rec;
+        if (raw.m != 0.f) {
+          RnRecord rec = rn_make_record(raw, Xc, Yc);
+          m4 = rn_subblock_mask(rec) & live_sb;
+          rec.d.x = __uint_as_float(m4);
+          if (m4) buf[lane] = rec;
+        }
       }
       // gather of the next batch and id load of the one after, in flight during the blend loop
       if (base + 32 + lane < n) rn_stage_issue(stage, lane, id_nxt, means2d, conic_opacity, rgb, masks);
@@ -84,30 +92,34 @@ __global__ void __launch_bounds__(RN_THREADS, RN_FWD_MINB) render_fwd_kernel(
         todo &= todo - 1;
         const float4 ra = buf[jj].a, rb = buf[jj].b, rc = buf[jj].c;
         // the same record is read by every lane: a warp reduction hands the compiler that fact (uniform branches)
-        const uint32_t sb = __reduce_or_sync(0xffffffffu, __float_as_uint(rc.w)) & live_sb;
-        const float lo = rb.y, m = rb.z;
+        const uint32_t sb = __reduce_or_sync(0xffffffffu, __float_as_uint(buf[jj].d.x)) & live_sb;
+        const float hi = rb.z, cap = rb.w, m = rc.w;
         const uint32_t pos = (uint32_t)(base + jj + 1);
-        const RnPartial p = rn_partial(ra, rb, fx, fy);
-        {
+        const RnPartial p = rn_partial(ra, rb, L);
 #pragma unroll
-          for (int k = 0; k < 4; k++) {
-            if ((sb >> k) & 1u) {
-              const float e = rn_eval(p, ra.w, k);
-              const bool pass = rn_filter(e, lo) && ((live >> k) & 1u);
-              if (__any_sync(0xffffffffu, pass)) {
-                // branch-free inside the section: a pair that fails the filter blends with alpha = 0 (w = 0, T' = T)
-                const float alpha = pass ? fminf(MG_ALPHA_MAX, rn_ex2(e)) : 0.f;
-                const float a = m * alpha;
-                const float Tn = T[k] * (1.f - a);
-                const bool stop = pass && Tn < MG_T_MIN;  // this entry is not blended; pos - 1 entries were consumed
-                const float w = stop ? 0.f : a * T[k];
-                Cr[k] = fmaf(w, rc.x, Cr[k]);
-                Cg[k] = fmaf(w, rc.y, Cg[k]);
-                Cb[k] = fmaf(w, rc.z, Cb[k]);
-                T[k] = stop ? T[k] : Tn;
-                live = stop ? live & ~(1u << k) : live;
-                last[k] = stop ? pos - 1 : last[k];
-              }
+        for (int c = 0; c < 2; c++) {
+          if (sb & (5u << c)) {  // sub-block c or c + 2 reachable and live
+            const float2 e = rn_eval_pair(p, L, c);
+            const bool pass0 = rn_filter(e.x, hi) && pos <= last[c];
+            const bool pass1 = rn_filter(e.y, hi) && pos <= last[c + 2];
+            if (__any_sync(0xffffffffu, pass0 | pass1)) {
+              // branch-free inside the section: a pixel that fails the filter blends with alpha = 0 (w = 0, T' = T)
+              float2 alpha;
+              alpha.x = pass0 ? fminf(cap, rn_ex2(e.x)) : 0.f;
+              alpha.y = pass1 ? fminf(cap, rn_ex2(e.y)) : 0.f;
+              const float2 a = rn_mul2(rn_splat(m), alpha);
+              const float2 Tn = rn_fma2(make_float2(-a.x, -a.y), T[c], T[c]);  // T (1 - a)
+              const bool stop0 = pass0 && Tn.x < MG_T_MIN, stop1 = pass1 && Tn.y < MG_T_MIN;
+              float2 w = rn_mul2(a, T[c]);  // this entry is not blended if it stops the pixel; pos - 1 entries were consumed
+              w.x = stop0 ? 0.f : w.x;
+              w.y = stop1 ? 0.f : w.y;
+              Cr[c] = rn_fma2(w, rn_splat(rc.x), Cr[c]);
+              Cg[c] = rn_fma2(w, rn_splat(rc.y), Cg[c]);
+              Cb[c] = rn_fma2(w, rn_splat(rc.z), Cb[c]);
+              T[c].x = stop0 ? T[c].x : Tn.x;
+              T[c].y = stop1 ? T[c].y : Tn.y;
+              last[c] = stop0 ? pos - 1 : last[c];
+              last[c + 2] = stop1 ? pos - 1 : last[c + 2];
             }
           }
         }
@@ -116,7 +128,7 @@ __global__ void __launch_bounds__(RN_THREADS, RN_FWD_MINB) render_fwd_kernel(
       live_sb = 0;
 #pragma unroll
       for (int k = 0; k < 4; k++)
-        if (__any_sync(0xffffffffu, (live >> k) & 1u)) live_sb |= 1u << k;
+        if (__any_sync(0xffffffffu, last[k] == (uint32_t)n)) live_sb |= 1u << k;
       if (!live_sb) break;
     }
     rn_cp_async_wait_all();
@@ -126,12 +138,14 @@ __global__ void __launch_bounds__(RN_THREADS, RN_FWD_MINB) render_fwd_kernel(
 #pragma unroll
   for (int k = 0; k < 4; k++) {
     const int x = px[k & 1], y = py[k >> 1];
-    if (x < W && y < H) {
+    if (x < W && y < H) {  // (n_contrib of a pixel of an empty list: last = n = 0)
       const size_t pix = (size_t)y * W + x;
-      image[pix] = fmaf(T[k], bg0, Cr[k]);
-      image[plane + pix] = fmaf(T[k], bg1, Cg[k]);
-      image[2 * plane + pix] = fmaf(T[k], bg2, Cb[k]);
-      final_T[pix] = T[k];
+      const int c = k & 1;
+      const float Tk = (k >> 1) ? T[c].y : T[c].x;
+      image[pix] = fmaf(Tk, bg0, (k >> 1) ? Cr[c].y : Cr[c].x);
+      image[plane + pix] = fmaf(Tk, bg1, (k >> 1) ? Cg[c].y : Cg[c].x);
+      image[2 * plane + pix] = fmaf(Tk, bg2, (k >> 1) ? Cb[c].y : Cb[c].x);
+      final_T[pix] = Tk;
       n_contrib[pix] = last[k];
     }
   }

@@ -149,12 +149,12 @@ L2_CLEAN = 1e-4  # relative 2-norm error of a gradient array ove
 L2_ALL = 2e-3    # ... over every element: a flagged Gaussian may differ by whole alpha >= 1/255 contributions
 
 
-def grads_vs_ref(fr, ref, names, clean, max_flag_frac, l2_clean=L2_CLEAN, l2_all=L2_ALL):
+def grads_vs_ref(fr, ref, names, clean, max_flag_frac, l2_clean=L2_CLEAN, l2_all=L2_ALL, rtol=GRAD_RTOL, floor_frac=1e-5):
     """Elementwise on the non-flagged Gaussians (north_star: 1e-3 relative) + the two 2-norm bounds."""
     out = {}
     for k in names:
         g = f64(getattr(fr, k))
-        out[k] = round(grad_close(g, ref[k], k, mask=clean), 4)
+        out[k] = round(grad_close(g, ref[k], k, rtol=rtol, floor_frac=floor_frac, mask=clean), 4)
         nrm_c, nrm = np.linalg.norm(ref[k][clean]), np.linalg.norm(ref[k])
         if nrm_c > 0:
             out[k + "_l2clean"] = float(np.linalg.norm((g - ref[k])[clean]) / nrm_c)
