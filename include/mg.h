@@ -191,6 +191,41 @@ size_t mg_render_loss_workspace_bytes(int32_t width, int32_t height);
 int mg_render_loss(int32_t width, int32_t height, const float* image, const float* target, float lambda_dssim,
                    float* dL_dimage, double* stats, void* workspace, size_t workspace_bytes, void* stream);
 
+/* ---- Density-control statistics and the optimiser step.  The paper keeps "the densification
+ * scheme" and the training procedure of the 3DGS method it modifies and prints neither; DESIGN.md
+ * readings 27-28 state what is computed.
+ *
+ * mg_density_stats (reading 27), after mg_render_bwd of a view: for every Gaussian with radii[i] > 0 (visible in it)
+ *   grad_accum[i] += sqrt((scale_x g_x)^2 + (scale_y g_y)^2), g = dL_dmeans2d[i] (pixels, reading 19);
+ *   denom[i] += 1;  max_radii[i] = max(max_radii[i], radii[i]).
+ * grad_accum, denom, max_radii: [N] fp32, UPDATED IN PLACE (the caller zeroes them when a densification step has consumed
+ * them); Gaussians with radii[i] == 0 are neither read nor written.  (scale_x, scale_y) = (1, 1) keeps pixel units;
+ * (W/2, H/2) gives the normalised-device-coordinate units of the 3DGS lineage's thresholds. */
+int mg_density_stats(int64_t N, const float* dL_dmeans2d, const int32_t* radii, float scale_x, float scale_y,
+                     float* grad_accum, float* denom, float* max_radii, void* stream);
+
+/* mg_adam_step (reading 28): Adam (Kingma & Ba 2015, Algorithm 1, bias-corrected) over up to MG_ADAM_MAX_GROUPS attribute
+ * groups in ONE launch, each with its own learning rate:
+ *   m <- beta1 m + (1 - beta1) g;  v <- beta2 v + (1 - beta2) g^2;
+ *   p <- p - lr (m / (1 - beta1^step)) / (sqrt(v / (1 - beta2^step)) + eps),   step = 1, 2, ...
+ * groups_host: HOST array of n_groups descriptors of DEVICE arrays with n_rows * row_floats floats each (16-byte aligned);
+ * param, m, v are UPDATED IN PLACE, grad is read only.  fp32 state and arithmetic (IEEE sqrt and division).
+ * radii (DEVICE, may be NULL): if given, every group must have one row per Gaussian (n_rows = N) and the rows of Gaussians
+ * with radii[i] == 0 are left untouched -- parameter and both moments (the variant that skips Gaussians not visible in the
+ * view, whose gradient is exactly zero).  NULL = every element is updated. */
+#define MG_ADAM_MAX_GROUPS 8
+typedef struct {
+  float* param;
+  const float* grad;
+  float* m;
+  float* v;
+  int64_t n_rows;
+  int32_t row_floats; /* 1..1024 */
+  float lr;
+} mg_adam_group;
+int mg_adam_step(int32_t n_groups, const mg_adam_group* groups_host, float beta1, float beta2, float eps, int64_t step,
+                 const int32_t* radii, void* stream);
+
 /* ---- Measurement aid (the FP32 roofline of the blend kernels needs a measured peak; the driver's
  * MEASURED_PEAKS.json has none).  Runs dependent-free FMA chains on every SM for at least min_seconds per instruction
  * form and times them with CUDA events; SYNCHRONOUS (returns when the measurement is done).

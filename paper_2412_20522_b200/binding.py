@@ -35,7 +35,7 @@ class mg_camera(C.Structure):
 EXPORTS = ["mg_last_error_string", "mg_version", "mg_workspace_bytes", "mg_preprocess", "mg_bin_sort",
            "mg_render_fwd", "mg_render_bwd", "mg_preprocess_bwd", "mg_mask_sample", "mg_mask_sample_bwd", "mg_mask_loss",
            "mg_mask_prune_keep", "mg_compact_workspace_bytes", "mg_compact", "mg_render_loss_workspace_bytes",
-           "mg_render_loss", "mg_measure_fp32_peak", "mg_debug_set_lookback_spin_limit"]
+           "mg_render_loss", "mg_density_stats", "mg_adam_step", "mg_measure_fp32_peak", "mg_debug_set_lookback_spin_limit"]
 
 
 def lib():
@@ -205,6 +205,31 @@ def mg_render_loss(image, target, lambda_dssim, dL_dimage, stats, workspace):
     _check(lib().mg_render_loss(C.c_int32(W), C.c_int32(H), _ptr(image, F32), _ptr(target, F32), C.c_float(lambda_dssim),
                                 _ptr(dL_dimage, F32), _ptr(stats, torch.float64), _ptr(workspace, U8),
                                 C.c_size_t(workspace.numel()), _stream()))
+
+
+def mg_density_stats(dL_dmeans2d, radii, scale, grad_accum, denom, max_radii):
+    N = radii.shape[0]
+    _check(lib().mg_density_stats(C.c_int64(N), _ptr(dL_dmeans2d, F32), _ptr(radii, I32), C.c_float(scale[0]),
+                                  C.c_float(scale[1]), _ptr(grad_accum, F32), _ptr(denom, F32), _ptr(max_radii, F32),
+                                  _stream()))
+
+
+class mg_adam_group(C.Structure):
+    _fields_ = [("param", C.c_void_p), ("grad", C.c_void_p), ("m", C.c_void_p), ("v", C.c_void_p),
+                ("n_rows", C.c_int64), ("row_floats", C.c_int32), ("lr", C.c_float)]
+
+
+def mg_adam_step(groups, beta1, beta2, eps, step, radii=None):
+    """groups: list of (param, grad, m, v, lr) with contiguous fp32 device tensors of one shape [n_rows, ...] each."""
+    arr = (mg_adam_group * max(len(groups), 1))()
+    for k, (p, g, m, v, lr) in enumerate(groups):
+        for t in (p, g, m, v):
+            assert t.is_contiguous() and t.dtype == F32 and t.device.type == "cuda" and t.shape == p.shape
+        n_rows = p.shape[0]
+        arr[k].param, arr[k].grad, arr[k].m, arr[k].v = p.data_ptr(), g.data_ptr(), m.data_ptr(), v.data_ptr()
+        arr[k].n_rows, arr[k].row_floats, arr[k].lr = n_rows, (p.numel() // n_rows if n_rows else 1), float(lr)
+    _check(lib().mg_adam_step(C.c_int32(len(groups)), arr, C.c_float(beta1), C.c_float(beta2), C.c_float(eps),
+                              C.c_int64(step), _ptr(radii, I32), _stream()))
 
 
 def mg_measure_fp32_peak(min_seconds=0.05):

@@ -15,7 +15,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libmg.so")
-SOURCES = ["api.cu", "preprocess.cu", "binsort.cu", "render_fwd.cu", "render_bwd.cu", "preprocess_bwd.cu", "maskhead.cu", "renderloss.cu", "peak.cu"]
+SOURCES = ["api.cu", "preprocess.cu", "binsort.cu", "render_fwd.cu", "render_bwd.cu", "preprocess_bwd.cu", "maskhead.cu", "renderloss.cu", "optimizer.cu", "peak.cu"]
 HEADERS = ["mg_common.cuh", "render_common.cuh"]
 
 

@@ -125,3 +125,22 @@ def test_invalid_arguments_of_the_next_rows_are_rejected_without_a_gpu(lib):
     assert binding.mg_render_loss_workspace_bytes(10, 5) == 9 * 4 * 50
     rc = lib.mg_render_loss(C.c_int32(10), C.c_int32(5), null, null, C.c_float(0.2), null, null, null, C.c_size_t(0), null)
     assert rc == binding.MG_ERR_INVALID_ARG
+
+
+def test_invalid_arguments_of_f4_are_rejected_without_a_gpu(lib):
+    """Density statistics and the optimiser step: argument checks happen before any CUDA call."""
+    from paper_2412_20522_b200 import binding
+
+    null = C.c_void_p(0)
+    rc = lib.mg_density_stats(C.c_int64(10), null, null, C.c_float(1.0), C.c_float(1.0), null, null, null, null)
+    assert rc == binding.MG_ERR_INVALID_ARG and b"null" in lib.mg_last_error_string()
+    assert lib.mg_density_stats(C.c_int64(0), null, null, C.c_float(1.0), C.c_float(1.0), null, null, null, null) == 0
+    grp = (binding.mg_adam_group * 1)()
+    grp[0].n_rows, grp[0].row_floats, grp[0].lr = 10, 3, 0.1
+    f = lambda *a: lib.mg_adam_step(*a)
+    assert f(C.c_int32(1), grp, C.c_float(0.9), C.c_float(0.999), C.c_float(1e-15), C.c_int64(1), null, null) == binding.MG_ERR_INVALID_ARG
+    assert b"null" in lib.mg_last_error_string()
+    assert f(C.c_int32(1), grp, C.c_float(0.9), C.c_float(0.999), C.c_float(1e-15), C.c_int64(0), null, null) == binding.MG_ERR_INVALID_ARG
+    assert f(C.c_int32(1), grp, C.c_float(1.0), C.c_float(0.999), C.c_float(1e-15), C.c_int64(1), null, null) == binding.MG_ERR_INVALID_ARG
+    assert f(C.c_int32(9), grp, C.c_float(0.9), C.c_float(0.999), C.c_float(1e-15), C.c_int64(1), null, null) == binding.MG_ERR_INVALID_ARG
+    assert f(C.c_int32(0), null, C.c_float(0.9), C.c_float(0.999), C.c_float(1e-15), C.c_int64(1), null, null) == 0
