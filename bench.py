@@ -8,8 +8,9 @@ value = Gaussian-pixel blends per second (forward + backward blends of the frame
 oracle/work_counts.json, divided by the device time of a whole step), inputs resident in HBM.
 e2e    = the same with host buffers: pinned-host -> device copies of every input and device -> host reads
          of the image and all gradients inside the timed region.
-roofline = the dominant kernel (largest share of the step), FP32-ALU bound, against the FP32 peak
-         derived in DESIGN.md (148 SMs x 128 lanes x 2 flop x sm_max_mhz).
+roofline = the dominant kernel (largest share of the step), FP32-ALU bound, against the FP32 peak measured on this
+         chip by mg_measure_fp32_peak (the figure derived from the unit counts is printed beside it); `rooflines` has
+         one entry per C-ABI call (HBM-bound calls against MEASURED_PEAKS.json's copy bandwidth).
 cpu_baseline / --impl reference = the oracle, as it stands, on the host cores, on a bounded sample of tiles.
 N > 1: one process per GPU (torchrun), replicas only -- no collective on the data path.
 """
@@ -27,17 +28,42 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-# algorithmic flops (counted once from the oracle's O10/O11 arithmetic)
-FLOP_PAIR = 13        # per pair evaluation: 2 sub, 6 quadratic form, mul, min, 2 compares (+1 MUFU not counted)
-FLOP_BLEND_FWD = 11   # per blend, forward
-FLOP_BLEND_BWD = 59   # per blend, backward (49 + 10 adds of the per-entry reduction)
-# dram__bytes_read.sum + dram__bytes_write.sum per launch at config 3, from the `ncu --set full` capture summarised
-# in profiles/r01z_final.md (the report itself is not committed); null for other configs
-NCU_TRAFFIC_BYTES = {3: {"render_bwd": 916.3e6 + 122.3e6, "render_fwd": 297.4e6 + 20.4e6}}
-# kernels of libmg launched per step (memsets and copies not counted): bin_sort = depth keys + ctl + 4 single-kernel
-# radix passes + row expansion (count, 2 scan, plan, emit) + column expansion (count, 2 scan, emit, ranges, tile order)
+# Algorithmic work per unit -- the ONE place these constants live (counted once from the oracle's
+# O10/O11 arithmetic).  Work the method does not require is not charged: under reading 5 the forward pass never looks
+# at an entry with M = 0, and the backward pass owes such an entry dL/dM only.
+FLOP_PAIR = 13             # per pair evaluation: 2 sub, 6 quadratic form, mul, min, 2 compares (+1 MUFU not counted)
+FLOP_BLEND_FWD = 11        # per unmasked blend, forward: M alpha, T' (fma), compare, a T, 3 fma
+FLOP_BLEND_BWD = 59        # per unmasked blend, backward (49 + 10 adds of the per-entry reduction)
+FLOP_BLEND_BWD_MASKED = 12  # per masked blend, backward: g.c (5), g.c - g.b, T x, alpha X accumulate (2), its reduction add, 2 compares
+BYTES_PRE = (301, 109)     # mg_preprocess, per visible / per culled Gaussian
+BYTES_PRE_BWD = (513, 240)  # mg_preprocess_bwd, per visible / per culled Gaussian
+BYTES_SORT_KEY = 25        # mg_bin_sort, per duplicated key, this scheme; the floor of any scheme is 4
+# dram__bytes_read.sum + dram__bytes_write.sum per launch, summed over the kernels of each call: written by
+# `python -m paper_2412_20522_b200.ncu_summary` from the `ncu --set full` capture named in profiles/r02_final.md
+TRAFFIC_JSON = os.path.join(ROOT, "profiles", "r02_traffic.json")
+# kernels of libmg launched per step (memsets and copies not counted), see binsort.cu for the sort's list
 KERNELS_PER_STEP = {"preprocess": 1, "bin_sort": 2 + 4 + 5 + 6, "render_fwd": 1, "render_bwd": 1,
                     "preprocess_bwd": 2}
+
+
+def ncu_traffic(cfg):
+    """{call: bytes per launch} for this config from the tracked ncu summary, or {} if there is none."""
+    if not os.path.exists(TRAFFIC_JSON):
+        return {}
+    return json.load(open(TRAFFIC_JSON)).get(str(cfg), {})
+
+
+def algorithmic_work(wc, N):
+    """Per call: (bound, work per launch, unit).  Flops for the blend kernels, bytes for the HBM-bound calls."""
+    vis, cul = wc["visible"], N - wc["visible"]
+    fwd_flop = ((wc["fwd_pair_evals"] - wc["fwd_pair_evals_masked"]) * FLOP_PAIR
+                + (wc["fwd_blends"] - wc["fwd_blends_masked"]) * FLOP_BLEND_FWD)
+    bwd_flop = (wc["bwd_pair_evals"] * FLOP_PAIR + (wc["bwd_blends"] - wc["bwd_blends_masked"]) * FLOP_BLEND_BWD
+                + wc["bwd_blends_masked"] * FLOP_BLEND_BWD_MASKED)
+    return {"preprocess": ("hbm", vis * BYTES_PRE[0] + cul * BYTES_PRE[1]),
+            "bin_sort": ("hbm", wc["R"] * BYTES_SORT_KEY),
+            "render_fwd": ("alu", fwd_flop), "render_bwd": ("alu", bwd_flop),
+            "preprocess_bwd": ("hbm", vis * BYTES_PRE_BWD[0] + cul * BYTES_PRE_BWD[1])}
 
 
 def work_counts(cfg):
@@ -57,7 +83,7 @@ class ClockSampler:
         self.proc = None
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                          "-i", str(index), "-lms", "50"], stdout=subprocess.PIPE, text=True)
+                                          "-i", str(index), "-lms", "20"], stdout=subprocess.PIPE, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
         except OSError:
@@ -305,6 +331,43 @@ def bench_render_loss(sc, hbm_gbs, reps=30):
             "note": "13 MB per plane set: L2-resident, launch- and latency-bound at this size"}
 
 
+def bench_optimizer(sc, g, fr, hbm_gbs, reps=10):
+    """SURVEY.md 8(f) row f4 at the bench workload's N: the statistics after a backward pass and one fused Adam step
+    over the 59 floats per Gaussian + 2 mask scores (28 B per parameter float: p, g, m, v in; p, m, v out), dense and
+    restricted to the Gaussians visible in the view."""
+    import torch
+
+    from paper_2412_20522_b200 import binding as mg
+
+    n = sc.N
+    scores = torch.zeros(n, 2, device="cuda")
+    params = [g["means"].clone(), g["log_scales"].clone(), g["quats"].clone(), g["opacity_logits"].clone(), g["sh"].clone(), scores]
+    grads = [fr.dL_dmeans, fr.dL_dlog_scales, fr.dL_dquats, fr.dL_dopacity_logits, fr.dL_dsh, torch.zeros_like(scores)]
+    groups = [(p, gr, torch.zeros_like(p), torch.zeros_like(p), 1e-4) for p, gr in zip(params, grads)]
+    acc, den, mxr = (torch.zeros(n, device="cuda") for _ in range(3))
+    nfl = sum(p.numel() for p in params)
+    vis = int((fr.radii > 0).sum())
+    calls = {"adam_step": (lambda: mg.mg_adam_step(groups, 0.9, 0.999, 1e-15, 3), 28 * nfl),
+             "adam_step_visible_only": (lambda: mg.mg_adam_step(groups, 0.9, 0.999, 1e-15, 3, fr.radii), 28 * (nfl // n) * vis + 4 * n),
+             "density_stats": (lambda: mg.mg_density_stats(fr.dL_dmeans2d, fr.radii, (1.0, 1.0), acc, den, mxr), 4 * n + 32 * vis)}
+    out = {"N": n, "visible": vis, "param_floats": nfl, "ms": {}, "gb_per_s": {}, "frac_of_hbm_peak": {}}
+    for name, (fn, nbytes) in calls.items():
+        for _ in range(2):
+            fn()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(reps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / reps
+        out["ms"][name] = round(ms, 4)
+        out["gb_per_s"][name] = round(nbytes / (ms * 1e-3) / 1e9, 1)
+        out["frac_of_hbm_peak"][name] = round(nbytes / (ms * 1e-3) / 1e9 / hbm_gbs, 3)
+    return out
+
+
 def n_threads():
     try:
         return len(os.sched_getaffinity(0))
@@ -354,7 +417,18 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--all-cameras", action="store_true", help="also time every camera of the scene (config 5: 20)")
+    ap.add_argument("--no-config5", action="store_true", help="skip the config 5 (20 cameras) entry of next_rows")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # started as `python bench.py --gpus N`: become N ranks, one per GPU (replicas)
+        import socket
+
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        os.execv(sys.executable, [sys.executable, "-m", "torch.distributed.run", "--nnodes=1",
+                                  f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1", "--master-port", str(port),
+                                  os.path.abspath(__file__)] + sys.argv[1:])
     rank = int(os.environ.get("RANK", 0))
     world = int(os.environ.get("WORLD_SIZE", 1))
     local = int(os.environ.get("LOCAL_RANK", 0))
@@ -510,37 +584,50 @@ def main():
     value = world * blends / (ms_step * 1e-3) if blends else None
     e2e_value = world * blends / (e2e_ms * 1e-3) if blends else None
 
-    # ---- roofline of the dominant kernel
-    dom = max(("render_fwd", "render_bwd"), key=lambda n: per_call[n])
+    # ---- rooflines: every call against the peak that bounds it; `roofline` = the dominant kernel's entry
     peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    sm_max = 1965.0
-    if os.path.exists(peaks_path):
-        sm_max = float(json.load(open(peaks_path)).get("sm_max_mhz", sm_max))
+    peaks = json.load(open(peaks_path)) if os.path.exists(peaks_path) else {}
+    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+    hbm_gbs = float(peaks.get("hbm_gbs", 6540.8))
+    hbm_source = "MEASURED_PEAKS.json hbm_gbs (copy, burst)" if "hbm_gbs" in peaks else "fallback of B200_PROFILING.md"
     fp32_derived = 148 * 128 * 2 * sm_max * 1e6 / 1e12  # TFLOP/s from the guide's unit counts (context)
     fp32_meas = mg.mg_measure_fp32_peak(0.05)             # timed on this chip, now (MEASURED_PEAKS.json has no FP32 entry)
     fp32_peak = max(fp32_meas["ffma_sustained"], fp32_meas["ffma2_sustained"])
-    roofline = None
+    roofline, rooflines = None, None
     if wc:
-        if dom == "render_bwd":
-            flops = wc["bwd_pair_evals"] * FLOP_PAIR + wc["bwd_blends"] * FLOP_BLEND_BWD
-        else:
-            flops = wc["fwd_pair_evals"] * FLOP_PAIR + wc["fwd_blends"] * FLOP_BLEND_FWD
-        ach = flops / (per_call[dom] * 1e-3) / 1e12
-        roofline = {"kernel": dom + "_kernel", "bound": "alu", "achieved": ach, "peak": fp32_peak, "unit": "TFLOP/s",
-                    "frac": ach / fp32_peak,
-                    "traffic": NCU_TRAFFIC_BYTES.get(args.config, {}).get(dom), "traffic_unit": "bytes per launch (ncu, profiles/r01z_final.md)",
-                    "flop_per_launch": flops, "share_of_step": per_call[dom] / sum(per_call.values()),
-                    "peak_source": "measured: mg_measure_fp32_peak, dependent-free FMA chains on every SM, >= 50 ms, sustained",
-                    "peak_measured": fp32_meas, "peak_derived": fp32_derived}
+        traffic = ncu_traffic(args.config)
+        rooflines = {}
+        tot = sum(per_call.values())
+        for call, (bound, work) in algorithmic_work(wc, sc.N).items():
+            sec = per_call[call] * 1e-3
+            if bound == "alu":
+                ach, peak, unit = work / sec / 1e12, fp32_peak, "TFLOP/s"
+            else:
+                ach, peak, unit = work / sec / 1e9, hbm_gbs, "GB/s"
+            rooflines[call] = {"bound": bound, "achieved": ach, "peak": peak, "unit": unit, "frac": ach / peak,
+                               "traffic": traffic.get(call), "work_per_launch": work, "ms": per_call[call],
+                               "share_of_step": per_call[call] / tot}
+        dom = max(("render_fwd", "render_bwd"), key=lambda n: per_call[n])
+        survey = wc[dom[7:] + "_pair_evals"] * FLOP_PAIR + wc[dom[7:] + "_blends"] * (FLOP_BLEND_BWD if dom == "render_bwd" else FLOP_BLEND_FWD)
+        roofline = dict(rooflines[dom], kernel=dom + "_kernel",
+                        traffic_unit="bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum, profiles/r02_final.md)",
+                        flop_per_launch=rooflines[dom]["work_per_launch"],
+                        flop_counting="masked and unmasked work charged separately (bench.py FLOP_*, DESIGN.md 7.6)",
+                        frac_by_survey_constants=survey / (per_call[dom] * 1e-3) / 1e12 / fp32_peak,
+                        peak_source="measured: mg_measure_fp32_peak, dependent-free FMA chains on every SM, >= 50 ms, sustained",
+                        peak_measured=fp32_meas, peak_derived=fp32_derived, hbm_peak_source=hbm_source)
 
-    hbm_gbs = 6540.8
-    if os.path.exists(peaks_path):
-        hbm_gbs = float(json.load(open(peaks_path)).get("hbm_gbs", hbm_gbs))
-    next_rows = {"mask_head": bench_mask_head(sc, g, hbm_gbs), "inference": bench_inference(sc, g, m),
-                 "render_loss": bench_render_loss(sc, hbm_gbs)} if world == 1 else None
-
-    if args.all_cameras and world == 1 and next_rows is not None:
-        next_rows["all_cameras"] = bench_cameras(sc, g, m)
+    next_rows = None
+    if world == 1:
+        next_rows = {"mask_head": bench_mask_head(sc, g, hbm_gbs), "inference": bench_inference(sc, g, m),
+                     "render_loss": bench_render_loss(sc, hbm_gbs), "optimizer": bench_optimizer(sc, g, fr, hbm_gbs)}
+        if args.all_cameras:
+            next_rows["all_cameras"] = bench_cameras(sc, g, m)
+        if args.config == 3 and not args.no_config5:
+            # BASELINE.json configs[4]: "Forward+backward are timed over 20 cameras on a circle" -- in the default record
+            sc5 = scenes.make(5)
+            g5, m5 = mg.upload(sc5)
+            next_rows["config5"] = dict(bench_cameras(sc5, g5, m5, steps=5), workload=workload_name(5).replace(", camera 0", ", its 20 cameras"))
 
     cpu = None
     if not args.no_cpu_baseline:
@@ -561,7 +648,8 @@ def main():
             "e2e": {"value": e2e_value, "unit": "blends/s", "ms_per_step": e2e_ms, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "how": "pinned host buffers; H2D of all inputs and D2H of image + all gradients every step, software-pipelined over 3 streams and 2 buffer sets",
                     "ms_per_step_unpipelined": e2e_serial_ms},
-            "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu, "next_rows": next_rows}
+            "gpu_launches": launches, "roofline": roofline, "rooflines": rooflines, "cpu_baseline": cpu,
+            "next_rows": next_rows}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

@@ -57,3 +57,33 @@ def test_reference_arm_prints_one_line_from_rank0_only():
     assert d["impl"] == "reference" and d["n_gpus"] == 2
     assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["value"] == d["value"]
     assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["e2e"]["d2h_bytes_per_step"] == 0
+
+
+def test_gpus_flag_alone_starts_the_ranks():
+    """`python bench.py --gpus 2` WITHOUT torchrun (the way a user, or a driver, may start it) must become 2 ranks:
+    bench.py re-executes itself under torch.distributed.run.  Checked on the reference arm (CPU): rank 0 prints the
+    line with n_gpus = 2, the spawned rank 1 exits 0 silently."""
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    env["OMP_NUM_THREADS"] = "2"
+    r = subprocess.run([sys.executable, "bench.py", "--impl", "reference", "--gpus", "2", "--steps", "1", "--warmup", "1",
+                        "--config", "1"], cwd=ROOT, env=env, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1, r.stdout
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["n_gpus"] == 2
+
+
+def test_algorithmic_work_charges_masked_and_unmasked_separately():
+    """bench.py's roofline numerators from the oracle's split counters: forward charges nothing for
+    masked entries (reading 5), backward charges a masked blend dL/dM only."""
+    sys.path.insert(0, ROOT)
+    import bench
+
+    wc = dict(visible=70, R=1000, fwd_pair_evals=500, fwd_pair_evals_masked=200, fwd_blends=50, fwd_blends_masked=20,
+              bwd_pair_evals=480, bwd_pair_evals_masked=190, bwd_blends=48, bwd_blends_masked=19)
+    w = bench.algorithmic_work(wc, 100)
+    assert w["render_fwd"] == ("alu", 300 * bench.FLOP_PAIR + 30 * bench.FLOP_BLEND_FWD)
+    assert w["render_bwd"] == ("alu", 480 * bench.FLOP_PAIR + 29 * bench.FLOP_BLEND_BWD + 19 * bench.FLOP_BLEND_BWD_MASKED)
+    assert w["preprocess"] == ("hbm", 70 * 301 + 30 * 109) and w["preprocess_bwd"] == ("hbm", 70 * 513 + 30 * 240)
+    assert w["bin_sort"] == ("hbm", 1000 * bench.BYTES_SORT_KEY)
