@@ -192,3 +192,32 @@ def check_preprocess_bwd(fr, sc, cam):
         rel = np.linalg.norm((g - ref[k])[vis]) / max(nrm, 1e-300)
         out[k + "_l2"] = float(rel)
     return ref, out
+
+
+def check_adam_step(got, ref, p_before, g, lr, beta1, beta2, eps, step, name=""):
+    """(p', m', v') of mg_adam_step against the oracle's, tolerances derived from the kernel's fp32 arithmetic
+    (e = 2^-24; every operation of csrc/optimizer.cu adam_one is one correctly rounded IEEE operation):
+
+    m' = fma(beta1, m, fl(fl(1 - beta1) g)): the constant, the product and the fma are rounded once each, so
+        |dm'| <= e (2 |(1 - beta1) g| + |m'|).
+      The bound is relative to the TERMS, not to the result: beta1 m and (1 - beta1) g have either sign and can cancel; a
+      bound relative to m' alone fails there (0.26 % of the elements of the test distribution, on the GPU and in an fp32
+      numpy emulation alike) although nothing is wrong.
+    v' = fma(beta2, v, fl(fl(fl(1 - beta2) g) g)): both terms are >= 0, nothing cancels: |dv'| <= 4.5 e v' < 4e-7 v'.
+    p' = fl(p - u), u = fl(fl(step_size m') / denom), denom = fma(fl(sqrt v'), c, eps):
+        |dp'| <= |du/dm'| |dm'| + 9.3 e |u| + e |p'|,   du/dm' = step_size / denom.
+      The first term matters where m' cancelled while v' is small (the tests draw m and v independently of g); without it
+      4 elements in 5.4 M of the emulation exceed the bound.  Used as 1e-6 |u| + 1.2e-7 |p'| + 1.1 x the first term.
+    """
+    e = 2.0 ** -24
+    (p_got, m_got, v_got), (p_ref, m_ref, v_ref) = got, ref
+    g = np.asarray(g, np.float64)
+    bc1, bc2 = 1.0 - beta1 ** step, 1.0 - beta2 ** step
+    dm = 1.1 * e * (2.0 * np.abs((1.0 - beta1) * g) + np.abs(m_ref))
+    bad = np.abs(np.asarray(m_got, np.float64) - m_ref) > dm + 1e-37
+    assert not bad.any(), (name, "first moment", int(bad.sum()), "of", bad.size)
+    np.testing.assert_allclose(v_got, v_ref, rtol=4e-7, atol=1e-37, err_msg=name)
+    u = np.abs(p_ref - np.asarray(p_before, np.float64))
+    du_dm = (lr / bc1) / (np.sqrt(v_ref / bc2) + eps)
+    bad = np.abs(np.asarray(p_got, np.float64) - p_ref) > 1e-6 * u + 1.2e-7 * np.abs(p_ref) + du_dm * dm + 1e-30
+    assert not bad.any(), (name, "parameter", int(bad.sum()), "of", bad.size)
