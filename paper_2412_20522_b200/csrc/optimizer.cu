@@ -21,6 +21,7 @@ struct AdamGroupDev {
   unsigned int row_floats;
   float step_size;           // lr / (1 - beta1^t)
   unsigned int block_begin;  // first block of this group
+  unsigned int rf_magic;     // ceil(2^32 / row_floats) (0 if row_floats == 1): floor(x / row_floats) = umulhi(x, magic) for x < 2^16
 };
 struct AdamParams {
   AdamGroupDev grp[MG_ADAM_MAX_GROUPS];
@@ -45,7 +46,13 @@ __global__ void __launch_bounds__(OP_THREADS) adam_kernel(const __grid_constant_
   const AdamGroupDev& G = P.grp[gi];
   const unsigned long long base = (unsigned long long)(blockIdx.x - G.block_begin) * OP_FLOATS_PER_BLOCK;
   const float step_size = G.step_size;
-  const bool small = G.total < (1ull << 32);  // 32-bit row arithmetic
+  // Row of an element (kRows): ONE division per block -- the block's first element is base = row0 * row_floats + rem0 --
+  // and from there the in-block offset x = rem0 + (element - base) < 4096 + 1024 is divided by a multiply-high with the
+  // host's reciprocal, exact for x row_floats < 2^32.  When row_floats is a multiple of 4 a vector lies within one row.
+  const unsigned int rf = G.row_floats, magic = G.rf_magic;
+  const unsigned long long row0 = kRows ? base / rf : 0ull;
+  const unsigned int rem0 = kRows ? (unsigned int)(base - row0 * rf) : 0u;
+  const bool vec_in_row = (rf & 3u) == 0u;
 
   unsigned long long e[OP_VEC_PER_THREAD];
   unsigned int vis[OP_VEC_PER_THREAD];  // bit j: element e + j is to be updated
@@ -57,12 +64,17 @@ __global__ void __launch_bounds__(OP_THREADS) adam_kernel(const __grid_constant_
       const unsigned int nvalid = (unsigned int)min(4ull, G.total - e[k]);
       vis[k] = (1u << nvalid) - 1u;
       if (kRows) {
+        const unsigned int x = rem0 + 4u * (unsigned int)(k * OP_THREADS + threadIdx.x);
         unsigned int mbits = 0;
+        if (vec_in_row) {
+          if (radii[row0 + __umulhi(x, magic)] > 0) mbits = vis[k];
+        } else {
 #pragma unroll
-        for (unsigned int j = 0; j < 4; j++) {
-          if (j < nvalid) {
-            const unsigned long long row = small ? (unsigned long long)((unsigned int)(e[k] + j) / G.row_floats) : (e[k] + j) / G.row_floats;
-            if (radii[row] > 0) mbits |= 1u << j;
+          for (unsigned int j = 0; j < 4; j++) {
+            if (j < nvalid) {
+              const unsigned int r = magic ? __umulhi(x + j, magic) : x + j;
+              if (radii[row0 + r] > 0) mbits |= 1u << j;
+            }
           }
         }
         vis[k] = mbits;
@@ -168,6 +180,7 @@ extern "C" int mg_adam_step(int32_t n_groups, const mg_adam_group* groups_host, 
     d.p = g.param; d.g = g.grad; d.m = g.m; d.v = g.v;
     d.total = (unsigned long long)g.n_rows * (unsigned long long)g.row_floats;
     d.row_floats = (unsigned int)g.row_floats;
+    d.rf_magic = g.row_floats == 1 ? 0u : (unsigned int)(((1ull << 32) + (unsigned long long)g.row_floats - 1) / (unsigned long long)g.row_floats);
     d.step_size = (float)((double)g.lr / bc1);
     d.block_begin = (unsigned int)blocks;
     blocks += (d.total + OP_FLOATS_PER_BLOCK - 1) / OP_FLOATS_PER_BLOCK;

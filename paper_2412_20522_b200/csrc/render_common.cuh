@@ -107,6 +107,16 @@ __device__ __forceinline__ void rn_stage_issue(RnStage* s, int lane, uint32_t id
   rn_cp_async(&s->m[lane], masks + id, 4);
 }
 
+// The same without the mask (the forward kernel has it already when it gathers the attributes).
+__device__ __forceinline__ void rn_stage_issue_attr(RnStage* s, int lane, uint32_t id, const float2* __restrict__ means2d,
+                                                    const float4* __restrict__ conic_opacity, const float* __restrict__ rgb) {
+  rn_cp_async(&s->co[lane], conic_opacity + id, 16);
+  rn_cp_async(&s->m2[lane], means2d + id, 8);
+  rn_cp_async(&s->rgb[lane][0], rgb + 3 * (size_t)id, 4);
+  rn_cp_async(&s->rgb[lane][1], rgb + 3 * (size_t)id + 1, 4);
+  rn_cp_async(&s->rgb[lane][2], rgb + 3 * (size_t)id + 2, 4);
+}
+
 __device__ __forceinline__ RnRaw rn_stage_read(const RnStage* s, int lane) {
   RnRaw v;
   v.m2 = s->m2[lane];

@@ -4,15 +4,17 @@
 //
 // FP32-issue bound (no dense contraction on this path, so no tensor cores).  Design (render_common.cuh):
 //  * 2 independent warps per tile, each a 16x8 strip of four 8x4 sub-blocks, one pixel of each per lane;
-//  * per warp, 32 list entries at a time: attributes gathered one batch ahead (cp.async), the record of the entry
-//    expanded about the strip's centre and a 4-bit sub-block reach mask per entry (lanes = entries), a ballot, then the
-//    surviving entries in list order;
+//  * an entry with M = 0 changes neither C nor T and cannot stop a pixel, and n_contrib counts the
+//    entries consumed before the stop (include/mg.h, reading 5), so the forward pass owes masked entries nothing.  They
+//    are removed BEFORE anything expensive happens: the warp classifies its list 64 entries at a time -- ids from a
+//    register prefetch, only the 4-byte mask of each entry gathered (cp.async) -- and a ballot appends the survivors'
+//    (id, list position, M) to a small ring queue in shared memory;
+//  * the attributes are gathered (cp.async, one batch ahead) for full batches of 32 UNMASKED entries taken from the
+//    queue; each lane expands its entry's record about the strip's centre and computes its 4-bit sub-block reach mask
+//    (lanes = entries), a ballot, then the surviving entries are walked in list order;
 //  * per surviving entry only the reachable, still-live pairs of sub-blocks are evaluated, two pixels per packed
 //    FP32 instruction; the alpha filter is two compares on the exponent, the exponential is taken only for pixels
 //    that pass;
-//  * an entry with M = 0 changes neither C nor T and cannot stop a pixel, and n_contrib counts
-//    the entries consumed before the stop (include/mg.h, reading 5), so masked entries are dropped when the
-//    batch is staged: the forward pass costs nothing for them;
 //  * a warp leaves when all its pixels have stopped.
 #include "render_common.cuh"
 
@@ -22,6 +24,30 @@
 
 namespace {
 
+// Per-warp ring queue of the list's unmasked entries that have not been turned into records yet, and the landing
+// zone of one classification step.  A step never finds more than 31 entries waiting (a full batch would have been
+// taken first) and adds at most FQ_STEP, so FQ_CAP = 128 slots are never overrun.
+constexpr int FQ_STEP = 64;
+constexpr int FQ_CAP = 128;
+struct FwdQueue {
+  uint32_t id[FQ_CAP];
+  uint32_t pos[FQ_CAP];  // 1-based position in the tile's list
+  float m[FQ_CAP];
+  uint32_t rid[FQ_STEP];  // ids of the step whose masks are in flight
+  float land[FQ_STEP];    // its masks (cp.async)
+};
+
+__device__ __forceinline__ RnRaw rn_stage_read_attr(const RnStage* s, int lane) {
+  RnRaw v;
+  v.m2 = s->m2[lane];
+  v.co = s->co[lane];
+  v.r = s->rgb[lane][0];
+  v.g = s->rgb[lane][1];
+  v.b = s->rgb[lane][2];
+  v.m = 0.f;
+  return v;
+}
+
 __global__ void __launch_bounds__(RN_THREADS, RN_FWD_MINB) render_fwd_kernel(
     int W, int H, int gw, float bg0, float bg1, float bg2, const uint32_t* __restrict__ sorted_ids,
     const uint2* __restrict__ tile_ranges, const uint32_t* __restrict__ tile_order,
@@ -29,11 +55,13 @@ __global__ void __launch_bounds__(RN_THREADS, RN_FWD_MINB) render_fwd_kernel(
     const float* __restrict__ masks, float* __restrict__ image, float* __restrict__ final_T, uint32_t* __restrict__ n_contrib) {
   __shared__ RnRecord buf_all[RN_WARPS][32];
   __shared__ RnStage stage_all[RN_WARPS];
+  __shared__ FwdQueue queue_all[RN_WARPS];
   const int tile = tile_order ? (int)tile_order[blockIdx.x] : (int)blockIdx.x;  // longest lists first
   const int tx = tile % gw, ty = tile / gw;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   RnRecord* buf = buf_all[warp];
   RnStage* stage = &stage_all[warp];
+  FwdQueue* Q = &queue_all[warp];
   const uint2 range = tile_ranges[tile];
   const int n = (int)(range.y - range.x);
   const uint32_t* ids = sorted_ids + range.x;
@@ -62,29 +90,81 @@ __global__ void __launch_bounds__(RN_THREADS, RN_FWD_MINB) render_fwd_kernel(
     if (__any_sync(0xffffffffu, last[k] != 0u)) live_sb |= 1u << k;
 
   if (n > 0 && live_sb) {
-    // prologue: gather of batch 0 in flight, ids of batch 1 in a register
-    if (lane < n) rn_stage_issue(stage, lane, ids[lane], means2d, conic_opacity, rgb, masks);
-    rn_cp_async_commit();
-    uint32_t id_nxt = 32 + lane < n ? ids[32 + lane] : 0u;
+    // ---- classification of the list, FQ_STEP entries per step (two per lane)
+    int rnext = 0;         // first list position (0-based) of the next step to be issued
+    int rland = -1;        // first list position of the step whose masks are in flight / have landed (-1: none)
+    int qhead = 0, qcount = 0;  // ring queue of unmasked entries not yet turned into records
+    uint32_t idA = lane < n ? ids[lane] : 0u, idB = 32 + lane < n ? ids[32 + lane] : 0u;  // ids of step rnext
+    // the masks of a step are gathered into Q->land; its ids are kept beside them until the step is classified
+    auto issue_step = [&]() {
+      Q->rid[lane] = idA;
+      Q->rid[32 + lane] = idB;
+      if (rnext + lane < n) rn_cp_async(&Q->land[lane], masks + idA, 4);
+      if (rnext + 32 + lane < n) rn_cp_async(&Q->land[32 + lane], masks + idB, 4);
+      rland = rnext;
+      rnext += FQ_STEP;
+      idA = rnext + lane < n ? ids[rnext + lane] : 0u;  // ids of the step after, in flight until that step is issued
+      idB = rnext + 32 + lane < n ? ids[rnext + 32 + lane] : 0u;
+    };
+    auto classify_step = [&]() {  // the step at rland has landed
+      const int p0 = rland + lane, p1 = rland + 32 + lane;
+      const float m0 = p0 < n ? Q->land[lane] : 0.f, m1 = p1 < n ? Q->land[32 + lane] : 0.f;
+      const uint32_t b0 = __ballot_sync(0xffffffffu, m0 != 0.f), b1 = __ballot_sync(0xffffffffu, m1 != 0.f);
+      const uint32_t lt = (1u << lane) - 1u;
+      const int tail = qhead + qcount;
+      if (m0 != 0.f) {
+        const int s = (tail + __popc(b0 & lt)) & (FQ_CAP - 1);
+        Q->id[s] = Q->rid[lane]; Q->pos[s] = (uint32_t)(p0 + 1); Q->m[s] = m0;
+      }
+      if (m1 != 0.f) {
+        const int s = (tail + __popc(b0) + __popc(b1 & lt)) & (FQ_CAP - 1);
+        Q->id[s] = Q->rid[32 + lane]; Q->pos[s] = (uint32_t)(p1 + 1); Q->m[s] = m1;
+      }
+      qcount += __popc(b0) + __popc(b1);
+      rland = -1;
+      __syncwarp();  // queue entries visible to the lanes that will gather them; land / rid free for the next step
+    };
+    // Fills the queue to a full batch (or to the end of the list), issues the attribute gather of the next batch (its
+    // size is returned) and keeps the mask gather of one step in flight.  Only the first step classified here can
+    // have been in flight already; a further one costs a round trip, which other warps cover.  Invariant: at most ONE
+    // step is issued and not yet classified (rland >= 0), because rid / land hold exactly one step.
+    auto refill_and_issue = [&]() -> int {
+      while (qcount < 32 && (rland >= 0 || rnext < n)) {
+        if (rland < 0) issue_step();
+        rn_cp_async_commit();
+        rn_cp_async_wait_all();
+        __syncwarp();
+        classify_step();
+      }
+      const int nb = min(32, qcount);
+      if (lane < nb) rn_stage_issue_attr(stage, lane, Q->id[(qhead + lane) & (FQ_CAP - 1)], means2d, conic_opacity, rgb);
+      // one more step of masks in flight -- unless one is still waiting to be classified (the queue was full enough
+      // without it): its ids and landing zone must not be overwritten
+      if (rland < 0 && rnext < n) issue_step();
+      rn_cp_async_commit();
+      return nb;
+    };
 
-    for (int base = 0; base < n; base += 32) {
-      rn_cp_async_wait_all();  // this lane's entry of the current batch has landed
+    int nb = refill_and_issue();  // prologue: batch 0 in flight
+    while (nb > 0) {
+      rn_cp_async_wait_all();  // this lane's entry of the current batch has landed (and the masks of the step in flight)
       __syncwarp();            // every lane is done reading the previous batch's records
       uint32_t m4 = 0;
-      if (base + lane < n) {
-        const RnRaw raw = rn_stage_read(stage, lane);
-        // an entry with M = 0 changes neither C nor T and cannot stop a pixel: dropped here
-        if (raw.m != 0.f) {
-          RnRecord rec = rn_make_record(raw, Xc, Yc);
-          m4 = rn_subblock_mask(rec) & live_sb;
-          rec.d.x = __uint_as_float(m4);
-          if (m4) buf[lane] = rec;
-        }
+      if (lane < nb) {
+        const int s = (qhead + lane) & (FQ_CAP - 1);
+        RnRaw raw = rn_stage_read_attr(stage, lane);
+        raw.m = Q->m[s];
+        RnRecord rec = rn_make_record(raw, Xc, Yc);
+        m4 = rn_subblock_mask(rec) & live_sb;
+        rec.d.x = __uint_as_float(m4);
+        rec.d.w = __uint_as_float(Q->pos[s]);  // 1-based list position (the record's 1/o slot: unused by the forward pass)
+        if (m4) buf[lane] = rec;
       }
-      // gather of the next batch and id load of the one after, in flight during the blend loop
-      if (base + 32 + lane < n) rn_stage_issue(stage, lane, id_nxt, means2d, conic_opacity, rgb, masks);
-      rn_cp_async_commit();
-      id_nxt = base + 64 + lane < n ? ids[base + 64 + lane] : 0u;
+      qhead = (qhead + nb) & (FQ_CAP - 1);
+      qcount -= nb;
+      __syncwarp();  // this batch's queue slots have been read by every lane before classification reuses any
+      // next batch: queue refill, attribute gather, one more step of masks -- all in flight during the blend loop
+      nb = refill_and_issue();
       __syncwarp();  // records visible to the whole warp
       uint32_t todo = __ballot_sync(0xffffffffu, m4 != 0);
       while (todo) {
@@ -94,7 +174,7 @@ __global__ void __launch_bounds__(RN_THREADS, RN_FWD_MINB) render_fwd_kernel(
         // the same record is read by every lane: a warp reduction hands the compiler that fact (uniform branches)
         const uint32_t sb = __reduce_or_sync(0xffffffffu, __float_as_uint(buf[jj].d.x)) & live_sb;
         const float hi = rb.z, cap = rb.w, m = rc.w;
-        const uint32_t pos = (uint32_t)(base + jj + 1);
+        const uint32_t pos = __float_as_uint(buf[jj].d.w);  // the entry's position in the tile's list
         const RnPartial p = rn_partial(ra, rb, L);
 #pragma unroll
         for (int c = 0; c < 2; c++) {

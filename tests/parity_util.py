@@ -104,7 +104,7 @@ def check_bin_sort(fr, cam):
     return ids_ref, ranges_ref
 
 
-def check_render_fwd(fr, cam, masks, ids, ranges, cut=CUT_STAGED, max_flag_frac=0.02, tiles=None):
+def check_render_fwd(fr, cam, masks, ids, ranges, cut=CUT_STAGED, max_flag_frac=1e-3, tiles=None):
     """Stage 3, staged: oracle blend on the GPU's fp32 splats and lists."""
     got = gpu_pre(fr)
     ref = orc.render_fwd(cam, ids, ranges, got["means2d"], got["conic_opacity"], got["rgb"], masks)
@@ -168,7 +168,7 @@ def grads_vs_ref(fr, ref, names, clean, max_flag_frac, l2_clean=L2_CLEAN, l2_all
     return out
 
 
-def check_render_bwd(fr, cam, N, masks, ids, ranges, dL_dimage, cut=CUT_STAGED, max_flag_frac=0.2):
+def check_render_bwd(fr, cam, N, masks, ids, ranges, dL_dimage, cut=CUT_STAGED, max_flag_frac=0.15):
     """Stage 4, staged."""
     got = gpu_pre(fr)
     ref = orc.render_bwd(cam, N, ids, ranges, got["means2d"], got["conic_opacity"], got["rgb"], masks,

@@ -29,7 +29,7 @@ def _need_gpu():
 # inputs: the rounding of two stages compounds, so the elementwise bound is twice north_star's 1e-3 (which the staged
 # comparison of each call holds on its own) and the absolute floor is 1e-4 of the array's largest element.
 E2E_GRAD_RTOL = 2e-3
-E2E_GRAD_BUDGET = {"tiny": 0.0, "cfg1": 0.2, "cfg2": 0.5, "cfg3_small": 0.2, "cfg4_small": 0.2}
+E2E_GRAD_BUDGET = {"tiny": 0.0, "cfg1": 0.14, "cfg2": 0.5, "cfg3_small": 0.08, "cfg4_small": 0.07}
 # Scenes whose END-TO-END comparison is ill-posed in fp32 and is therefore held in the 2-norm only.  "needles": the conic
 # that mg_preprocess stores is fp32 (relative rounding 6e-8 per component); at a pixel thousands of pixels from the
 # centre of a long thin splat the terms A dx^2, B dx dy, C dy^2 reach 1e4..1e6 and cancel, so that rounding alone moves
@@ -164,8 +164,9 @@ def test_unmasked_equals_all_ones(oracle):
     fr, *_ = pu.run_gpu(sc, masks=ones)
     cam = sc.camera
     ids, ranges = pu.check_bin_sort(fr, cam)
-    pu.check_render_fwd(fr, cam, ones, ids, ranges)
-    pu.check_render_bwd(fr, cam, sc.N, ones, ids, ranges, sc.dL_dimage())
+    _, s3 = pu.check_render_fwd(fr, cam, ones, ids, ranges, max_flag_frac=0.02)
+    _, s4 = pu.check_render_bwd(fr, cam, sc.N, ones, ids, ranges, sc.dL_dimage(), max_flag_frac=0.2)
+    print("PARITY", "cfg1 all-ones masks", dict(render_fwd=s3, render_bwd=s4))
 
 
 def test_fractional_masks(oracle):
@@ -175,8 +176,9 @@ def test_fractional_masks(oracle):
     fr, *_ = pu.run_gpu(sc, masks=m)
     cam = sc.camera
     ids, ranges = pu.check_bin_sort(fr, cam)
-    pu.check_render_fwd(fr, cam, m, ids, ranges)
-    pu.check_render_bwd(fr, cam, sc.N, m, ids, ranges, sc.dL_dimage())
+    _, s3 = pu.check_render_fwd(fr, cam, m, ids, ranges, max_flag_frac=0.02)
+    _, s4 = pu.check_render_bwd(fr, cam, sc.N, m, ids, ranges, sc.dL_dimage(), max_flag_frac=0.2)
+    print("PARITY", "cfg2 20k fractional masks", dict(render_fwd=s3, render_bwd=s4))
 
 
 def test_background_colour(oracle):
@@ -185,8 +187,36 @@ def test_background_colour(oracle):
     fr, *_ = pu.run_gpu(sc)
     cam = sc.camera
     ids, ranges = pu.check_bin_sort(fr, cam)
-    pu.check_render_fwd(fr, cam, sc.masks, ids, ranges)
-    pu.check_render_bwd(fr, cam, sc.N, sc.masks, ids, ranges, sc.dL_dimage())
+    _, s3 = pu.check_render_fwd(fr, cam, sc.masks, ids, ranges, max_flag_frac=0.02)
+    _, s4 = pu.check_render_bwd(fr, cam, sc.N, sc.masks, ids, ranges, sc.dL_dimage(), max_flag_frac=0.2)
+    print("PARITY", "cfg1 background colour", dict(render_fwd=s3, render_bwd=s4))
+
+
+@pytest.mark.parametrize("degree", [1, 2])
+def test_sh_degrees_1_and_2(oracle, degree):
+    """The configs use SH degree 0 and 3 only; mg_preprocess / mg_preprocess_bwd have one kernel instance per degree, and
+    degree 1 (48-byte rows: bulk copies) and degree 2 (108-byte rows: not a multiple of 16, loads by flat position) take
+    different staging paths.  config 2's geometry, N ragged against a warp and a block, higher bands strong enough to
+    clamp channels; the whole path is run, projection and projection backward are compared (staged)."""
+    import dataclasses
+
+    base = scenes.config2()
+    n = 20_011
+    sh = scenes._sh(np.random.default_rng(70 + degree), n, degree, 0.5, 0.3)
+    sc = dataclasses.replace(base, name=f"cfg2_sh{degree}", means=base.means[:n], log_scales=base.log_scales[:n],
+                             quats=base.quats[:n], opacity_logits=base.opacity_logits[:n], sh=sh, masks=base.masks[:n],
+                             cameras=[dataclasses.replace(base.camera, sh_degree=degree)])
+    fr, g, m, gimg = pu.run_gpu(sc)
+    cam = sc.camera
+    s1 = pu.check_preprocess(fr, sc, cam, max_flag_frac=0.02)
+    assert s1["n_clamped"] > 0, "the scene should clamp some channels"
+    ref5, s5 = pu.check_preprocess_bwd(fr, sc, cam)
+    vis = fr.radii.cpu().numpy() > 0
+    for k, v in s5.items():
+        assert v <= 1e-4, f"{k}: relative 2-norm error {v:.2e}"
+    for k in ref5:
+        pu.grad_close(pu.f64(getattr(fr, k))[vis], ref5[k][vis], k, rtol=1e-3, floor_frac=1e-4)
+    print("PARITY", sc.name, "staged", dict(preprocess=s1, preprocess_bwd=s5))
 
 
 def test_projection_backward_with_dense_upstream_gradients(oracle):
@@ -306,7 +336,8 @@ def test_huge_splat_covers_every_tile(oracle):
     gw, gh = mg.grid(sc.camera)
     assert (pu.u32(fr.tiles_touched)[:3] == gw * gh).all()
     ids, ranges = pu.check_bin_sort(fr, sc.camera)
-    pu.check_render_fwd(fr, sc.camera, sc.masks, ids, ranges)
+    _, s3 = pu.check_render_fwd(fr, sc.camera, sc.masks, ids, ranges, max_flag_frac=0.02)
+    print("PARITY", "cfg1 huge splats", dict(render_fwd=s3))
 
 
 def test_many_tiles_three_sort_passes(oracle):
