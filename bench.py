@@ -37,7 +37,7 @@ FLOP_BLEND_BWD = 59        # per unmasked blend, backward (49 + 10 adds of the p
 FLOP_BLEND_BWD_MASKED = 12  # per masked blend, backward: g.c (5), g.c - g.b, T x, alpha X accumulate (2), its reduction add, 2 compares
 BYTES_PRE = (301, 109)     # mg_preprocess, per visible / per culled Gaussian
 BYTES_PRE_BWD = (513, 240)  # mg_preprocess_bwd, per visible / per culled Gaussian
-BYTES_SORT_KEY = 25        # mg_bin_sort, per duplicated key, this scheme; the floor of any scheme is 4
+BYTES_SORT_KEY = 22        # mg_bin_sort, per duplicated key, this scheme; the floor of any scheme is 4
 # dram__bytes_read.sum + dram__bytes_write.sum per launch, summed over the kernels of each call: written by
 # `python -m paper_2412_20522_b200.ncu_summary` from the `ncu --set full` capture named in profiles/r02_final.md
 TRAFFIC_JSON = os.path.join(ROOT, "profiles", "r02_traffic.json")

@@ -4,9 +4,10 @@
 // The result is DEFINED as the ascending order of the 64-bit keys (tile_id << 32 | depth bits), ties
 // by Gaussian index, tile_id = ty * gw + tx.  It is produced without ever materialising those keys:
 //
-//  S1  depth order of the N Gaussians: stable LSD radix sort of the fp32 depth bits (4 x 8 bits).
+//  S1  depth order of the VISIBLE Gaussians: stable LSD radix sort of the fp32 depth bits (4 x 8 bits).
 //      All duplicates of a Gaussian share its depth, so the depth digits are sorted BEFORE the
-//      duplication (N keys instead of R).
+//      duplication (nvis keys instead of R).  The first pass reads depths and tiles_touched themselves and
+//      neither ranks nor writes a culled Gaussian, so the other three passes move the visible ones only.
 //  S2  row expansion: Gaussian k of the depth order covers tile rows [y0, y1); it emits one record
 //      (id, x0, x1) into the list of each of those rows, lists kept in depth order.  All duplicates
 //      of a Gaussian within a tile row share (depth, ty), so the row digit is "sorted" before the
@@ -123,32 +124,48 @@ std::atomic<int> g_spin_limit{LB_SPIN_LIMIT};             // mg_debug_set_lookba
 // offsets by summing the counts its predecessors have published (an "aggregate" if that tile has only
 // counted, an "inclusive" total -- which ends the walk -- once it has finished its own look-back).  Tiles
 // are taken in ticket order, so a block only ever waits for blocks that started before it.  The digit
-// bases of the whole array come from the histograms depth_keys_kernel took.
+// bases of the whole array come from the histograms depth_hist_kernel took.
+// kFirst (pass 0): keys_in = the fp32 depths of ALL n_all Gaussians, vals_in = their tiles_touched.  A Gaussian with
+// tiles_touched == 0 is neither ranked nor written (it is treated like an index past the end), its value is its index,
+// and the tile writes as many keys as it has visible Gaussians.  Tiles, tickets and the stable order are unchanged, so
+// the pass is at once the first digit pass and the compaction.  The other passes sort ctl->nvis keys; their grid is
+// sized for n_all and the surplus blocks leave at once.
+template <bool kFirst>
 __global__ void __launch_bounds__(RS_THREADS) radix_onesweep_kernel(
     const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in, uint32_t* __restrict__ keys_out,
-    uint32_t* __restrict__ vals_out, uint32_t n, int pass, SortCtl* __restrict__ ctl,
+    uint32_t* __restrict__ vals_out, uint32_t n_all, int pass, SortCtl* __restrict__ ctl,
     unsigned long long* __restrict__ status, int spin_limit) {
   extern __shared__ __align__(16) unsigned char rs_smem_raw[];
   RadixSmem& sm = *reinterpret_cast<RadixSmem*>(rs_smem_raw);
-  __shared__ uint32_t s_tile;
+  __shared__ uint32_t s_tile, s_nvalid;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int shift = 8 * pass;
+  const uint32_t n = kFirst ? n_all : ctl->nvis;
+  // exactly ceil(n / RS_TILE) blocks stay, and they take exactly the tickets below that number
+  if ((uint64_t)blockIdx.x * RS_TILE >= n) return;
   if (threadIdx.x == 0) s_tile = atomicAdd(&ctl->ticket[pass], 1u);
   for (int i = threadIdx.x; i < RS_WARPS * RS_BINS; i += RS_THREADS) (&sm.cnt[0][0])[i] = 0;
   __syncthreads();
   const uint32_t tile = s_tile;
   const uint32_t base = tile * (uint32_t)RS_TILE + warp * (32 * RS_ITEMS);
   uint32_t key[RS_ITEMS], val[RS_ITEMS], rank[RS_ITEMS];
+  uint32_t vbits = 0;  // bit it: this thread's item it takes part in the sort
 #pragma unroll
   for (int it = 0; it < RS_ITEMS; it++) {
     const uint32_t idx = base + it * 32 + lane;
-    key[it] = idx < n ? keys_in[idx] : 0u;
-    val[it] = (vals_in && idx < n) ? vals_in[idx] : idx;  // first pass: the value is the index itself
+    bool v = idx < n;
+    if (kFirst) {
+      v = v && vals_in[idx] != 0u;  // tiles_touched: culled Gaussians do not take part
+      val[it] = idx;                // the value is the Gaussian's index
+    } else {
+      val[it] = v ? vals_in[idx] : 0u;
+    }
+    key[it] = v ? keys_in[idx] : 0u;
+    vbits |= (v ? 1u : 0u) << it;
   }
 #pragma unroll
   for (int it = 0; it < RS_ITEMS; it++) {
-    const uint32_t idx = base + it * 32 + lane;
-    const bool valid = idx < n;
+    const bool valid = (vbits >> it) & 1u;
     const uint32_t d = (key[it] >> shift) & 255u;
     const uint32_t peers = peers_by_ballot(d, 8, __ballot_sync(0xffffffffu, valid));
     uint32_t before = 0;
@@ -187,6 +204,7 @@ __global__ void __launch_bounds__(RS_THREADS) radix_onesweep_kernel(
       for (int w = 0; w < RS_BINS / 32; w++)
         if (w < warp) woff += sm.gdelta[w];
       sm.lbase[threadIdx.x] = woff + inc - total;
+      if (threadIdx.x == RS_BINS - 1) s_nvalid = woff + inc;  // keys of this tile that take part
     }
     __syncthreads();
   }
@@ -210,8 +228,7 @@ __global__ void __launch_bounds__(RS_THREADS) radix_onesweep_kernel(
   // into digit order in shared memory
 #pragma unroll
   for (int it = 0; it < RS_ITEMS; it++) {
-    const uint32_t idx = base + it * 32 + lane;
-    if (idx < n) {
+    if ((vbits >> it) & 1u) {
       const uint32_t d = (key[it] >> shift) & 255u;
       const uint32_t lpos = sm.lbase[d] + sm.cnt[warp][d] + rank[it];
       sm.keys[lpos] = key[it];
@@ -219,7 +236,7 @@ __global__ void __launch_bounds__(RS_THREADS) radix_onesweep_kernel(
     }
   }
   __syncthreads();
-  const uint32_t nblk = min((uint32_t)RS_TILE, n - tile * (uint32_t)RS_TILE);
+  const uint32_t nblk = s_nvalid;
 #pragma unroll
   for (int it = 0; it < RS_ITEMS; it++) {
     const uint32_t j = it * RS_THREADS + threadIdx.x;
@@ -232,12 +249,14 @@ __global__ void __launch_bounds__(RS_THREADS) radix_onesweep_kernel(
   }
 }
 
-// Depth keys: fp32 bits of depth (positive floats order as unsigned ints); culled Gaussians last.
-// Also R = sum of tiles_touched, the number of visible Gaussians, and the digit histograms of all four
-// radix passes (they do not depend on the order of the keys, so one read of the keys gives all of them).
-__global__ void __launch_bounds__(256) depth_keys_kernel(int64_t N, const float* __restrict__ depths,
+// The sort key of a Gaussian is the fp32 bit pattern of its depth (positive floats order as unsigned ints); only
+// VISIBLE Gaussians (tiles_touched > 0) are sorted.  This kernel takes, in one read of depths and tiles_touched, the
+// digit histograms of all four radix passes over the visible keys (they do not depend on the order of the keys),
+// R = sum of tiles_touched and the number of visible Gaussians.  It writes no keys: the first radix pass reads the
+// depths itself.
+__global__ void __launch_bounds__(256) depth_hist_kernel(int64_t N, const float* __restrict__ depths,
                                                          const uint32_t* __restrict__ tiles_touched,
-                                                         uint32_t* __restrict__ keys, SortCtl* __restrict__ ctl) {
+                                                         SortCtl* __restrict__ ctl) {
   __shared__ unsigned long long s_sum[8];
   __shared__ uint32_t s_vis[8];
   __shared__ uint32_t hist[4][RS_BINS];
@@ -247,12 +266,13 @@ __global__ void __launch_bounds__(256) depth_keys_kernel(int64_t N, const float*
   uint32_t vis = 0;
   for (int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x; i < N; i += (int64_t)gridDim.x * 256) {
     const uint32_t tt = tiles_touched[i];
-    const uint32_t key = tt ? __float_as_uint(depths[i]) : 0xffffffffu;
-    keys[i] = key;
     sum += tt;
     vis += tt != 0;
+    if (tt) {
+      const uint32_t key = __float_as_uint(depths[i]);
 #pragma unroll
-    for (int p = 0; p < 4; p++) atomicAdd(&hist[p][(key >> (8 * p)) & 255u], 1u);
+      for (int p = 0; p < 4; p++) atomicAdd(&hist[p][(key >> (8 * p)) & 255u], 1u);
+    }
   }
 #pragma unroll
   for (int o = 16; o >= 1; o >>= 1) {
@@ -772,7 +792,8 @@ extern "C" int mg_bin_sort(const mg_camera* cam, int64_t N, const float* depths,
   int dev = 0, sms = 0;
   if (int rc = mg_current_device(&dev, &sms)) return rc;
   if (!attr_set.is_done(dev)) {
-    MG_CHECK_CUDA(cudaFuncSetAttribute(radix_onesweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(RadixSmem)));
+    MG_CHECK_CUDA(cudaFuncSetAttribute(radix_onesweep_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(RadixSmem)));
+    MG_CHECK_CUDA(cudaFuncSetAttribute(radix_onesweep_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(RadixSmem)));
     attr_set.set_done(dev);
   }
   const int dk_grid = sms * 8;
@@ -780,20 +801,24 @@ extern "C" int mg_bin_sort(const mg_camera* cam, int64_t N, const float* depths,
   MG_CHECK_CUDA(cudaMemsetAsync(status, 0, sizeof(unsigned long long) * 4 * (size_t)L.nblk_sort * RS_BINS, st));
   {
     const int64_t want = (N + 255) / 256;
-    depth_keys_kernel<<<(unsigned)(want < dk_grid ? want : dk_grid), 256, 0, st>>>(N, depths, tiles_touched, keysA, ctl);
+    depth_hist_kernel<<<(unsigned)(want < dk_grid ? want : dk_grid), 256, 0, st>>>(N, depths, tiles_touched, ctl);
   }
   ctl_finalize_kernel<<<1, RS_BINS, 0, st>>>(ctl, (unsigned long long)R_capacity);
   MG_CHECK_LAUNCH();
   {
-    uint32_t *ki = keysA, *vi = nullptr, *ko = keysB, *vo = valsB;
-    for (int pass = 0; pass < 4; pass++) {
-      radix_onesweep_kernel<<<L.nblk_sort, RS_THREADS, sizeof(RadixSmem), st>>>(
+    // pass 0 reads the caller's depths and tiles_touched and writes the visible (key, index) pairs to B; then B -> A -> B -> A
+    radix_onesweep_kernel<true><<<L.nblk_sort, RS_THREADS, sizeof(RadixSmem), st>>>(
+        reinterpret_cast<const uint32_t*>(depths), tiles_touched, keysB, valsB, (uint32_t)N, 0, ctl, status, spin_limit);
+    MG_CHECK_LAUNCH();
+    const uint32_t *ki = keysB, *vi = valsB;
+    uint32_t *ko = keysA, *vo = valsA;
+    for (int pass = 1; pass < 4; pass++) {
+      radix_onesweep_kernel<false><<<L.nblk_sort, RS_THREADS, sizeof(RadixSmem), st>>>(
           ki, vi, ko, vo, (uint32_t)N, pass, ctl, status + (size_t)pass * L.nblk_sort * RS_BINS, spin_limit);
       MG_CHECK_LAUNCH();
-      ki = (pass & 1) ? keysA : keysB;
-      vi = (pass & 1) ? valsA : valsB;
-      ko = (pass & 1) ? keysB : keysA;
-      vo = (pass & 1) ? valsB : valsA;
+      const uint32_t *tk = ki, *tv = vi;
+      ki = ko; vi = vo;
+      ko = const_cast<uint32_t*>(tk); vo = const_cast<uint32_t*>(tv);
     }
   }
   const uint32_t* order = valsA;  // after 4 passes the result is in (keysA, valsA)

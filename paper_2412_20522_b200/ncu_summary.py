@@ -24,7 +24,7 @@ COLS = [("Kernel Name", "kernel"), ("gpu__time_duration.sum", "time"), ("dram__b
         ("l1tex__throughput.avg.pct_of_peak_sustained_elapsed", "l1tex%")]
 
 CALL_OF = [("preprocess_bwd", "preprocess_bwd"), ("preprocess_kernel", "preprocess"), ("render_fwd", "render_fwd"),
-           ("render_bwd", "render_bwd"), ("depth_keys", "bin_sort"), ("ctl_", "bin_sort"), ("radix_", "bin_sort"),
+           ("render_bwd", "render_bwd"), ("depth_keys", "bin_sort"), ("depth_hist", "bin_sort"), ("ctl_", "bin_sort"), ("radix_", "bin_sort"),
            ("row_expand", "bin_sort"), ("col_expand", "bin_sort"), ("scan_", "bin_sort"), ("plan_", "bin_sort"),
            ("tile_ranges", "bin_sort"), ("tile_order", "bin_sort"), ("visible_", "bin_sort"), ("sort_", "bin_sort")]
 
