@@ -62,3 +62,13 @@ static inline int mg_grid_h(const mg_camera* c) { return (c->height + MG_TILE - 
 #define MG_SH_C3_4 -0.4570457994644658f
 #define MG_SH_C3_5 1.445305721320277f
 #define MG_SH_C3_6 -0.5900435899266435f
+
+// ---- asynchronous 16-byte copies global -> shared (LDGSTS): no registers are held while the data is in flight, so a
+// thread can have many more of them outstanding than loads into registers (.cg: the data is read once, keep it out of L1)
+#ifdef __CUDACC__
+__device__ __forceinline__ void mg_cp_async16(void* smem_dst, const void* gmem_src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void mg_cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void mg_cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+#endif

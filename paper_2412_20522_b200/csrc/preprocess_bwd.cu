@@ -121,12 +121,15 @@ __global__ void __launch_bounds__(PB_THREADS) preprocess_bwd_sh_kernel(
   // coalesced load of the visible rows
   if (nrows > 0) {
     if constexpr (L::VEC) {
+      // asynchronous copies, all of a lane's in flight at once (see mg_preprocess)
       const float4* src = reinterpret_cast<const float4*>(sh + g0 * RK);
 #pragma unroll
       for (int k = 0; k < RK / 4; k++) {
         const int f = k * 32 + lane, g = f / (RK / 4), c = f % (RK / 4);
-        if (g < nrows && ((vmask >> g) & 1u)) *reinterpret_cast<float4*>(wrow + g * STRIDE + 4 * c) = __ldg(src + f);
+        if (g < nrows && ((vmask >> g) & 1u)) mg_cp_async16(wrow + g * STRIDE + 4 * c, src + f);
       }
+      mg_cp_async_commit();
+      mg_cp_async_wait_all();
     } else {
       const float* src = sh + g0 * RK;
 #pragma unroll
