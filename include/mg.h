@@ -153,7 +153,10 @@ int mg_preprocess_bwd(const mg_camera* cam, int64_t N, const float* means, const
  *
  * mg_mask_sample (sec. 3.3: "we assign 2 learnable mask scores for each Gaussian, and apply Gumbel-Softmax
  * to sample one differentiable category out of the 2 scores, denoted M_i in {0,1}").  scores[N][2], uniforms[N][2] in
- * (0,1); g = -log(-log u); d = (s_1 + g_1) - (s_0 + g_0); masks[i] = 1 if d > 0 else 0 (category 1 = present, a tie
+ * (0,1).  A uniform outside the open interval -- generators on [0,1) return exactly 0, rounding to fp32 can give exactly
+ * 1 -- is taken as the nearest fp32 value inside it: u is clamped to [2^-126, 1 - 2^-24] (reading 29), so the
+ * noise lies in [-4.47, 16.64] and every output is finite; NaN uniforms are outside the contract.  The same holds for
+ * mg_mask_prune_keep.  g = -log(-log u); d = (s_1 + g_1) - (s_0 + g_0); masks[i] = 1 if d > 0 else 0 (category 1 = present, a tie
  * gives 0); soft[i] (may be NULL) = softmax((s + g) / tau)_1 = sigmoid(d / tau), kept for the backward pass.
  * tau > 0 is not stated in the paper (reading 22). */
 int mg_mask_sample(int64_t N, const float* scores, const float* uniforms, float tau, float* masks, float* soft,

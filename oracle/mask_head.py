@@ -14,6 +14,9 @@ reference [13] with a hard (one-hot) forward sample and the soft sample's deriva
 a tie (equal perturbed scores) gives M = 0.
 
   g_k   = -log(-log(u_k)),  u_k in (0,1)                       Gumbel(0,1) noise, k = 0, 1
+          (reading 29: a uniform outside the open interval -- fp32 generators on [0,1) return exactly 0 with probability
+          2^-24 per draw, and rounding to fp32 can give exactly 1 -- is taken as the nearest fp32 value inside it:
+          u is clamped to [2^-126, 1 - 2^-24], so g lies in [-4.47, 16.64] and d is always finite)
   d     = (s_1 + g_1) - (s_0 + g_0)
   y_1   = softmax((s + g)/tau)_1 = 1 / (1 + exp(-d / tau))      soft sample
   M     = 1 if d > 0 else 0                                     hard sample = argmax of the perturbed scores
@@ -28,8 +31,12 @@ from __future__ import annotations
 import numpy as np
 
 
+U_MIN = float(np.finfo(np.float32).tiny)                 # 2^-126, the smallest normal fp32
+U_MAX = float(np.float32(1.0) - np.float32(2.0 ** -24))  # 1 - 2^-24, the largest fp32 below 1
+
+
 def gumbel(u):
-    u = np.asarray(u, np.float64)
+    u = np.clip(np.asarray(u, np.float64), U_MIN, U_MAX)  # reading 29
     return -np.log(-np.log(u))
 
 

@@ -13,7 +13,11 @@ namespace {
 constexpr int MH_THREADS = 256;
 
 // d = (s_1 + g_1) - (s_0 + g_0) with g = -log(-log u): the hard sample is d > 0, the soft one sigmoid(d / tau).
+// A uniform outside (0,1) is taken as the nearest fp32 value inside it (include/mg.h, reading 29): the noise
+// stays within [-4.47, 16.64] and d is finite whatever the caller's generator returns at its endpoints.
 __device__ __forceinline__ float perturbed_gap(float2 s, float2 u) {
+  u.x = fminf(fmaxf(u.x, 1.17549435e-38f), 0.99999994f);
+  u.y = fminf(fmaxf(u.y, 1.17549435e-38f), 0.99999994f);
   // inner log accurate (for u near 1, -log u is tiny and needs its relative accuracy), outer log lg2-based
   const float g0 = -__logf(-logf(u.x)), g1 = -__logf(-logf(u.y));
   return (s.y + g1) - (s.x + g0);

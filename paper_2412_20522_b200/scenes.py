@@ -245,12 +245,12 @@ def make(config: int, **kw) -> Scene:
 
 def mask_head_inputs(n, seed=7, n_draws=10, score_sigma=2.0):
     """Seeded inputs of the mask head: 2 scores per Gaussian and the uniforms its samplers
-    consume (one draw for the training sample, n_draws for the prune rule).  No arithmetic of the method here:
-    the uniforms are clipped away from 0 and 1 so that log(-log u) is finite in fp32."""
+    consume (one draw for the training sample, n_draws for the prune rule).  No arithmetic of the method here, and
+    no narrowing of the inputs either: the fp32 cast of a uniform on [0,1) can be exactly 0 or exactly 1, and what
+    the samplers do with such a value is defined by the method's side (include/mg.h, reading 29)."""
     rng = np.random.default_rng(seed)
     scores = _f32(rng.normal(0.0, score_sigma, (n, 2)))
-    lo, hi = np.float32(1e-7), np.float32(1.0 - 6e-8)
-    u = np.clip(_f32(rng.uniform(0.0, 1.0, (n, 2))), lo, hi)
-    u_prune = np.clip(_f32(rng.uniform(0.0, 1.0, (n_draws, n, 2))), lo, hi)
+    u = _f32(rng.uniform(0.0, 1.0, (n, 2)))
+    u_prune = _f32(rng.uniform(0.0, 1.0, (n_draws, n, 2)))
     dL_dmask = _f32(rng.normal(0.0, 1.0, n))
     return scores, u, u_prune, dL_dmask

@@ -89,3 +89,30 @@ def test_compaction_edge_cases():
     mg.mg_compact(torch.empty(0, dtype=torch.uint8, device="cuda"), [], [], ws, n_out)
     torch.cuda.synchronize()
     assert int(n_out[0]) == 0
+
+
+def test_uniforms_at_and_beyond_the_endpoints():
+    """include/mg.h / DESIGN.md reading 29: a uniform outside (0,1) is taken as the nearest fp32 value inside it.  Every
+    pair of {0, 1, a denormal, 2^-126, 1 - 2^-24, a negative value, a value above 1} with ordinary ones, through
+    mg_mask_sample and mg_mask_prune_keep: finite outputs, and the oracle's hard and soft samples."""
+    special = np.array([0.0, 1.0, 1e-45, np.finfo(np.float32).tiny, 1.0 - 2.0 ** -24, -3.0, 7.0, 0.5, 0.013], np.float32)
+    a, b = np.meshgrid(special, special, indexing="ij")
+    u = np.stack([a.ravel(), b.ravel()], axis=1).astype(np.float32)
+    n = u.shape[0]
+    scores = np.random.default_rng(3).normal(0.0, 2.0, (n, 2)).astype(np.float32)
+    for tau in (1.0, 0.5):
+        ref = mh.sample(scores, u, tau)
+        masks, soft = torch.empty(n, device="cuda"), torch.empty(n, device="cuda")
+        mg.mg_mask_sample(dev(scores), dev(u), tau, masks, soft)
+        got_m, got_s = masks.cpu().numpy().astype(np.float64), soft.cpu().numpy().astype(np.float64)
+        assert np.isfinite(got_s).all() and np.isfinite(ref["soft"]).all()
+        ok = ref["margin"] > CUT
+        assert ok.sum() >= n - 2
+        assert np.array_equal(got_m[ok], ref["mask"][ok])
+        np.testing.assert_allclose(got_s, ref["soft"], atol=2e-5, rtol=0)
+    u10 = np.stack([np.roll(u, k, axis=0) for k in range(10)]).astype(np.float32)
+    keep_ref, margin = mh.prune_keep(scores, u10)
+    keep = torch.empty(n, dtype=torch.uint8, device="cuda")
+    mg.mg_mask_prune_keep(dev(scores), dev(u10), keep)
+    ok = margin > CUT
+    assert np.array_equal(keep.cpu().numpy().astype(bool)[ok], keep_ref[ok])

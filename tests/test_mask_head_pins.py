@@ -109,3 +109,27 @@ def test_compaction_is_stable_and_complete():
             assert out[2][j] == i and np.array_equal(out[0][j], arrays[0][i]) and np.array_equal(out[1][j], arrays[1][i])
             j += 1
     assert j == cnt
+
+
+def test_uniforms_at_and_beyond_the_endpoints():
+    """Reading 29: a uniform outside (0,1) is taken as the nearest fp32 value inside it, [2^-126, 1 - 2^-24].  Held against
+    the closed forms of the noise at those two values (not against the oracle's own clamp), and against what the
+    definition implies: values beyond the interval behave like its end, every output is finite, the noise is
+    non-decreasing in u, and a pair (0, 0) -- whose unclamped noise would be inf - inf -- gives the noise-free sample."""
+    g_lo = -np.log(126.0 * np.log(2.0))            # -ln(-ln 2^-126)
+    g_hi = -np.log(-np.log1p(-(2.0 ** -24)))       # -ln(-ln(1 - 2^-24))
+    assert mh.gumbel(0.0) == pytest.approx(g_lo, rel=1e-14) and mh.gumbel(1.0) == pytest.approx(g_hi, rel=1e-14)
+    assert -4.48 < g_lo < -4.46 and 16.63 < g_hi < 16.64
+    for beyond, end in ((-0.5, 0.0), (1e-45, 0.0), (-np.inf, 0.0), (1.5, 1.0), (np.inf, 1.0)):
+        assert mh.gumbel(beyond) == mh.gumbel(end)
+    u = np.array([0.0, 1e-45, np.finfo(np.float32).tiny, 1e-20, 0.25, 0.5, 0.75, 1.0 - 2.0 ** -24, 1.0])
+    g = mh.gumbel(u)
+    assert np.isfinite(g).all() and (np.diff(g) >= 0).all()
+    s = np.array([[0.3, -0.2], [1.0, 2.5]])
+    for pair in ((0.0, 0.0), (1.0, 1.0)):
+        r = mh.sample(s, np.tile(np.array(pair), (2, 1)), tau=0.7)
+        np.testing.assert_allclose(r["soft"], 1.0 / (1.0 + np.exp(-(s[:, 1] - s[:, 0]) / 0.7)), rtol=1e-14)
+        assert np.array_equal(r["mask"], (s[:, 1] > s[:, 0]).astype(np.float64))
+    # the extreme pairs decide the sample whatever the scores (|g_hi - g_lo| = 21.1 against scores of a few units)
+    assert mh.sample(s, np.tile(np.array((0.0, 1.0)), (2, 1)))["mask"].tolist() == [1.0, 1.0]
+    assert mh.sample(s, np.tile(np.array((1.0, 0.0)), (2, 1)))["mask"].tolist() == [0.0, 0.0]
