@@ -44,10 +44,21 @@ __global__ void __launch_bounds__(MH_THREADS) mask_sample_bwd_kernel(int64_t N, 
 }
 
 // stats[0] += sum of masks (double: exact for 0/1 masks whatever the order of the atomics)
-__global__ void __launch_bounds__(MH_THREADS) mask_sum_kernel(int64_t N, const float* __restrict__ masks, double* __restrict__ stats) {
+// L_m and its gradient in ONE kernel (two launches in round 1).  Every element needs the mean over all of them, so the
+// grid meets once: phase 1 sums the masks into stats[0]; a barrier; phase 2 adds lambda_m 2 mean / N to dL_dmask.  The
+// barrier is two counters kept in stats[1] and stats[2] (outputs that nobody reads before the end): blocks arrive, spin
+// until all have arrived, do phase 2, and leave; the block that leaves last overwrites the counters with the results,
+// when no block can be looking at them any more.  All blocks must be resident at once for the spin to end: the grid is
+// sized to that and the launch is cooperative, so the runtime refuses a grid that would not be.
+__global__ void __launch_bounds__(MH_THREADS) mask_loss_kernel(int64_t N, const float* __restrict__ masks, double lambda_m,
+                                                               float* __restrict__ dL_dmask, double* __restrict__ stats) {
   __shared__ double part[MH_THREADS / 32];
+  __shared__ double s_total;
+  unsigned long long* arrive = reinterpret_cast<unsigned long long*>(&stats[1]);
+  unsigned long long* leave = reinterpret_cast<unsigned long long*>(&stats[2]);
+  const int64_t stride = (int64_t)gridDim.x * MH_THREADS, first = (int64_t)blockIdx.x * MH_THREADS + threadIdx.x;
   double s = 0.0;
-  for (int64_t i = (int64_t)blockIdx.x * MH_THREADS + threadIdx.x; i < N; i += (int64_t)gridDim.x * MH_THREADS) s += (double)masks[i];
+  for (int64_t i = first; i < N; i += stride) s += (double)masks[i];
 #pragma unroll
   for (int o = 16; o >= 1; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
   if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = s;
@@ -57,16 +68,23 @@ __global__ void __launch_bounds__(MH_THREADS) mask_sum_kernel(int64_t N, const f
 #pragma unroll
     for (int w = 0; w < MH_THREADS / 32; w++) t += part[w];
     if (t != 0.0) atomicAdd(&stats[0], t);
+    __threadfence();
+    atomicAdd(arrive, 1ull);
+    while (*reinterpret_cast<volatile unsigned long long*>(arrive) < (unsigned long long)gridDim.x) {}
+    __threadfence();
+    s_total = *reinterpret_cast<volatile double*>(&stats[0]);
   }
-}
-
-// stats[1] = lambda_m (mean M)^2, stats[2] = mean M; dL_dmask[i] += lambda_m 2 mean / N
-__global__ void __launch_bounds__(MH_THREADS) mask_loss_apply_kernel(int64_t N, double lambda_m, double* __restrict__ stats,
-                                                                     float* __restrict__ dL_dmask) {
-  const double mean = stats[0] / (double)N;
-  const int64_t i = (int64_t)blockIdx.x * MH_THREADS + threadIdx.x;
-  if (i == 0) { stats[1] = lambda_m * mean * mean; stats[2] = mean; }
-  if (dL_dmask && i < N) dL_dmask[i] += (float)(lambda_m * 2.0 * mean / (double)N);
+  __syncthreads();
+  const double mean = s_total / (double)N;
+  if (dL_dmask) {
+    const float add = (float)(lambda_m * 2.0 * mean / (double)N);
+    for (int64_t i = first; i < N; i += stride) dL_dmask[i] += add;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0 && atomicAdd(leave, 1ull) == (unsigned long long)gridDim.x - 1) {
+    stats[1] = lambda_m * mean * mean;  // every block has left the spin: the counters are free
+    stats[2] = mean;
+  }
 }
 
 __global__ void __launch_bounds__(MH_THREADS) mask_prune_kernel(int64_t N, int S, const float2* __restrict__ scores,
@@ -167,9 +185,14 @@ extern "C" int mg_mask_loss(int64_t N, const float* masks, float lambda_m, float
   cudaStream_t st = (cudaStream_t)stream;
   MG_CHECK_CUDA(cudaMemsetAsync(stats, 0, 3 * sizeof(double), st));
   const int64_t want = (N + MH_THREADS - 1) / MH_THREADS;
-  mask_sum_kernel<<<(unsigned)(want < 1184 ? want : 1184), MH_THREADS, 0, st>>>(N, masks, stats);
-  mask_loss_apply_kernel<<<(unsigned)want, MH_THREADS, 0, st>>>(N, (double)lambda_m, stats, dL_dmask);
-  MG_CHECK_LAUNCH();
+  int sms = 0, per_sm = 0;
+  if (int rc = mg_current_device(nullptr, &sms)) return rc;
+  MG_CHECK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mask_loss_kernel, MH_THREADS, 0));
+  const int64_t resident = (int64_t)sms * (per_sm > 0 ? per_sm : 1);
+  const unsigned grid = (unsigned)(want < resident ? want : resident);
+  double lam = (double)lambda_m;
+  void* args[] = {(void*)&N, (void*)&masks, (void*)&lam, (void*)&dL_dmask, (void*)&stats};
+  MG_CHECK_CUDA(cudaLaunchCooperativeKernel((const void*)mask_loss_kernel, dim3(grid), dim3(MH_THREADS), args, 0, st));
   return MG_OK;
 }
 
