@@ -64,10 +64,13 @@ static inline int mg_grid_h(const mg_camera* c) { return (c->height + MG_TILE - 
 #define MG_SH_C3_6 -0.5900435899266435f
 
 // ---- asynchronous 16-byte copies global -> shared (LDGSTS): no registers are held while the data is in flight, so a
-// thread can have many more of them outstanding than loads into registers (.cg: the data is read once, keep it out of L1)
+// thread can have many more of them outstanding than loads into registers.  .ca (allocate at every level, like the loads
+// these copies replace), not .cg: with .cg the kernel itself was 4 us faster still, but the mg_preprocess that follows it
+// in the next frame ran 18 us slower (measured in the frame) -- what a kernel leaves in the caches is
+// part of its cost.
 #ifdef __CUDACC__
 __device__ __forceinline__ void mg_cp_async16(void* smem_dst, const void* gmem_src) {
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gmem_src) : "memory");
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gmem_src) : "memory");
 }
 __device__ __forceinline__ void mg_cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void mg_cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
