@@ -39,7 +39,7 @@ BYTES_PRE = (301, 109)     # mg_preprocess, per visible / per culled Gaussian
 BYTES_PRE_BWD = (513, 240)  # mg_preprocess_bwd, per visible / per culled Gaussian
 BYTES_SORT_KEY = 22        # mg_bin_sort, per duplicated key, this scheme; the floor of any scheme is 4
 # dram__bytes_read.sum + dram__bytes_write.sum per launch, summed over the kernels of each call: written by
-# `python -m paper_2412_20522_b200.ncu_summary` from the `ncu --set full` capture named in profiles/r02_final.md
+# `python -m paper_2412_20522_b200.ncu_summary` from the `ncu --set full` capture named in profiles/r02_final.md (section 3)
 TRAFFIC_JSON = os.path.join(ROOT, "profiles", "r02_traffic.json")
 # kernels of libmg launched per step (memsets and copies not counted), see binsort.cu for the sort's list
 KERNELS_PER_STEP = {"preprocess": 1, "bin_sort": 2 + 4 + 5 + 6, "render_fwd": 1, "render_bwd": 1,
