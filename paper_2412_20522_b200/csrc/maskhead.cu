@@ -139,16 +139,48 @@ __global__ void __launch_bounds__(CP_BLOCK) compact_pos_kernel(int64_t N, const 
   if (i < N) pos[i] = k ? block_offsets[blockIdx.x] + woff + __popc(ballot & ((1u << lane) - 1u)) : 0xffffffffu;
 }
 
-// One thread per input element (a float, or a float4 when the row size is a multiple of 4 floats): element e of an
-// array with r elements per row belongs to Gaussian e / r.  32-bit index arithmetic (the host checks the range).
-template <typename V>
-__global__ void __launch_bounds__(MH_THREADS) compact_rows_kernel(uint32_t n_elems, uint32_t r, const uint32_t* __restrict__ pos,
+// Input elements (a float, or a float4 when the row size is a multiple of 4 floats): element e of an array with r
+// elements per row belongs to Gaussian e / r.  CP_PER elements per thread, a block apart, all their loads issued before
+// any is stored (a copy is bound by the bytes in flight).  kR > 0: the row size is a compile-time constant, so the
+// division is a multiply (the sizes this method has: 1, 2, 3 and 12 elements per row); kR == 0: any r, a runtime
+// division.  32-bit index arithmetic (the host checks the range).
+constexpr int CP_PER = 4;
+template <typename V, int kR>
+__global__ void __launch_bounds__(MH_THREADS) compact_rows_kernel(uint32_t n_elems, uint32_t r_rt, const uint32_t* __restrict__ pos,
                                                                   const V* __restrict__ src, V* __restrict__ dst) {
-  const uint32_t e = blockIdx.x * (uint32_t)MH_THREADS + threadIdx.x;
-  if (e >= n_elems) return;
-  const uint32_t i = e / r;
-  const uint32_t p = pos[i];
-  if (p != 0xffffffffu) dst[(size_t)p * r + (e - i * r)] = src[e];
+  const uint32_t r = kR > 0 ? (uint32_t)kR : r_rt;
+  const uint32_t e0 = blockIdx.x * (uint32_t)(MH_THREADS * CP_PER) + threadIdx.x;
+  uint32_t p[CP_PER], j[CP_PER];
+#pragma unroll
+  for (int q = 0; q < CP_PER; q++) {
+    const uint32_t e = e0 + q * MH_THREADS;
+    p[q] = 0xffffffffu;
+    j[q] = 0;
+    if (e < n_elems) {
+      const uint32_t i = e / r;
+      j[q] = e - i * r;
+      p[q] = pos[i];
+    }
+  }
+  V v[CP_PER];
+#pragma unroll
+  for (int q = 0; q < CP_PER; q++)
+    if (p[q] != 0xffffffffu) v[q] = src[e0 + q * MH_THREADS];
+#pragma unroll
+  for (int q = 0; q < CP_PER; q++)
+    if (p[q] != 0xffffffffu) dst[(size_t)p[q] * r + j[q]] = v[q];
+}
+
+template <typename V>
+void compact_rows_launch(uint32_t ne, uint32_t r, const uint32_t* pos, const V* src, V* dst, cudaStream_t st) {
+  const unsigned grid = (unsigned)(((uint64_t)ne + MH_THREADS * CP_PER - 1) / (MH_THREADS * CP_PER));
+  switch (r) {
+    case 1: compact_rows_kernel<V, 1><<<grid, MH_THREADS, 0, st>>>(ne, r, pos, src, dst); break;
+    case 2: compact_rows_kernel<V, 2><<<grid, MH_THREADS, 0, st>>>(ne, r, pos, src, dst); break;
+    case 3: compact_rows_kernel<V, 3><<<grid, MH_THREADS, 0, st>>>(ne, r, pos, src, dst); break;
+    case 12: compact_rows_kernel<V, 12><<<grid, MH_THREADS, 0, st>>>(ne, r, pos, src, dst); break;
+    default: compact_rows_kernel<V, 0><<<grid, MH_THREADS, 0, st>>>(ne, r, pos, src, dst); break;
+  }
 }
 
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -241,10 +273,9 @@ extern "C" int mg_compact(int64_t N, const uint8_t* keep, int32_t n_arrays, cons
       const bool vec = row_floats[a] % 4 == 0 && ((uintptr_t)src[a] & 15) == 0 && ((uintptr_t)dst[a] & 15) == 0;
       const int64_t r = vec ? row_floats[a] / 4 : row_floats[a];
       const int64_t ne = N * r;
-      MG_REQUIRE(ne < ((int64_t)1 << 32) - MH_THREADS, "array too large for one compaction call (N * row size >= 2^32 elements)");
-      const unsigned grid = (unsigned)((ne + MH_THREADS - 1) / MH_THREADS);
-      if (vec) compact_rows_kernel<float4><<<grid, MH_THREADS, 0, st>>>((uint32_t)ne, (uint32_t)r, pos, (const float4*)src[a], (float4*)dst[a]);
-      else compact_rows_kernel<float><<<grid, MH_THREADS, 0, st>>>((uint32_t)ne, (uint32_t)r, pos, src[a], dst[a]);
+      MG_REQUIRE(ne < ((int64_t)1 << 32) - MH_THREADS * CP_PER, "array too large for one compaction call (N * row size >= 2^32 elements)");
+      if (vec) compact_rows_launch<float4>((uint32_t)ne, (uint32_t)r, pos, (const float4*)src[a], (float4*)dst[a], st);
+      else compact_rows_launch<float>((uint32_t)ne, (uint32_t)r, pos, src[a], dst[a], st);
     }
     MG_CHECK_LAUNCH();
   }
