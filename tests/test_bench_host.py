@@ -87,3 +87,25 @@ def test_algorithmic_work_charges_masked_and_unmasked_separately():
     assert w["render_bwd"] == ("alu", 480 * bench.FLOP_PAIR + 29 * bench.FLOP_BLEND_BWD + 19 * bench.FLOP_BLEND_BWD_MASKED)
     assert w["preprocess"] == ("hbm", 70 * 301 + 30 * 109) and w["preprocess_bwd"] == ("hbm", 70 * 513 + 30 * 240)
     assert w["bin_sort"] == ("hbm", 1000 * bench.BYTES_SORT_KEY)
+
+
+def test_roofline_traffic_is_what_the_tracked_ncu_capture_gives(tmp_path):
+    """bench.py's `roofline.traffic` comes from profiles/r02_traffic.json; that file must be exactly what
+    paper_2412_20522_b200.ncu_summary derives from the raw ncu CSV tracked beside it (the number was
+    a constant typed into bench.py and could go stale unnoticed), and every call of the hot path must be in it."""
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    raw = os.path.join(root, "profiles", "r02_ncu_raw.csv")
+    out = tmp_path / "traffic.json"
+    subprocess.check_call([sys.executable, "-m", "paper_2412_20522_b200.ncu_summary", raw, "--config", "3",
+                           "--md", str(tmp_path / "table.md"), "--traffic-json", str(out)], cwd=root)
+    derived = json.load(open(out))
+    tracked = json.load(open(os.path.join(root, "profiles", "r02_traffic.json")))
+    assert derived == tracked
+    assert set(tracked["3"]) == {"preprocess", "bin_sort", "render_fwd", "render_bwd", "preprocess_bwd"}
+    sys.path.insert(0, root)
+    import bench
+
+    assert bench.ncu_traffic(3) == tracked["3"]
+    # the table the same script writes has one row per kernel of a step: 22 launches
+    table = open(tmp_path / "table.md").read()
+    assert sum(1 for ln in table.splitlines() if ln.startswith("| ") and "_kernel" in ln) == 22
