@@ -21,6 +21,10 @@
  *     Calls may overlap on different streams, and be issued from different host threads, as long as they
  *     share no output or scratch buffer: the library keeps no device-side state of its own (every counter
  *     lives in caller memory) and its per-device one-time initialisations are thread-safe.
+ *   - Domain: finite inputs; quats need not be unit but |q|^2 must be a normal fp32 number (1e-19 < |q| < 1e19) --
+ *     a zero quaternion has no rotation, its covariance is not a number and the Gaussian is culled (radius 0, exact
+ *     zeros everywhere), and a norm that under- or overflows in fp32 behaves the same; exp(log_scale) and the projected
+ *     covariance must stay finite in fp32 (scales below ~1e15 pixels): beyond that the Gaussian is culled likewise.
  *   - Layouts: packed row-major fp32.  means[N][3], log_scales[N][3], quats[N][4] as (w,x,y,z),
  *     opacity_logits[N], sh[N][K][3] with K=(sh_degree+1)^2 (coefficient-major, RGB innermost),
  *     masks[N] (any real value; tests use {0,1}; Eq. 4 is affine in M), images planar [3][H][W].

@@ -437,3 +437,47 @@ def test_bin_sort_random_rects_through_the_c_abi(oracle, seed, W, H, n, big_frac
 
 def orc_bin_sort(oracle, cam, depths, rects, tt):
     return oracle.bin_sort(cam, depths, rects, tt)
+
+
+def test_degenerate_gaussians(oracle):
+    """The degenerate inputs the method has, mixed into config 1: a zero quaternion (its normalisation is 0/0: the
+    covariance is not a number and the Gaussian is culled, `det > 0` being false), vanishing scales (the covariance is
+    the 0.3 dilation alone), a very large scale (its rect covers the image), opacity logits of +-30 (opacity 1 -> the
+    0.99 clamp is active and cuts the gradient to the logit; opacity 1e-13 -> never passes the alpha filter), a centre
+    exactly on the near plane (z = 0.2: culled, the test is z > 0.2) and one behind the camera.  Staged parity of all
+    five calls, and no output of any call is non-finite."""
+    sc = scenes.config1()
+    n = sc.N
+    sc.quats[0] = 0.0
+    sc.log_scales[1] = -60.0
+    sc.log_scales[2] = [2.0, -60.0, 1.0]
+    sc.log_scales[3] = 3.0
+    sc.means[3] = [0.1, -0.1, 4.0]
+    sc.opacity_logits[3] = -2.0
+    sc.opacity_logits[4] = 30.0
+    sc.opacity_logits[5] = -30.0
+    sc.means[6] = [0.3, 0.2, 0.2]
+    sc.means[7] = [0.0, 0.0, -3.0]
+    sc.quats[8] = [0.0, 0.0, 0.0, 1e-15]  # tiny but inside the domain of include/mg.h (|q|^2 a normal fp32 number)
+    fr, g, m, gimg = pu.run_gpu(sc)
+    cam = sc.camera
+    radii = fr.radii.cpu().numpy()
+    assert radii[0] == 0 and radii[6] == 0 and radii[7] == 0, "zero quaternion, near plane and behind the camera are culled"
+    assert radii[1] > 0 and radii[3] > 0 and radii[8] > 0
+    gw, gh = mg.grid(cam)
+    assert pu.u32(fr.tiles_touched)[3] == gw * gh
+    for k in ("means2d", "depths", "conic_opacity", "rgb", "image", "final_T", "dL_dmeans2d", "dL_dconic", "dL_dopacity",
+              "dL_drgb", "dL_dmask", "dL_dmeans", "dL_dlog_scales", "dL_dquats", "dL_dopacity_logits", "dL_dsh"):
+        assert torch.isfinite(getattr(fr, k)).all(), k
+    s1 = pu.check_preprocess(fr, sc, cam, max_flag_frac=0.02)
+    ids, ranges = pu.check_bin_sort(fr, cam)
+    _, s3 = pu.check_render_fwd(fr, cam, sc.masks, ids, ranges)
+    _, s4 = pu.check_render_bwd(fr, cam, n, sc.masks, ids, ranges, sc.dL_dimage())
+    ref5, s5 = pu.check_preprocess_bwd(fr, sc, cam)
+    vis = radii > 0
+    for k, v in s5.items():
+        assert v <= 1e-4, f"{k}: relative 2-norm error {v:.2e}"
+    for k in ref5:
+        pu.grad_close(pu.f64(getattr(fr, k))[vis], ref5[k][vis], k, rtol=1e-3, floor_frac=1e-4)
+    assert float(fr.dL_dopacity_logits[4]) == 0.0 or abs(float(fr.dL_dopacity_logits[4])) < 1e-12, "sigmoid'(30) ~ 1e-13"
+    print("PARITY", "cfg1 degenerate Gaussians", dict(preprocess=s1, render_fwd=s3, render_bwd=s4, preprocess_bwd=s5))
