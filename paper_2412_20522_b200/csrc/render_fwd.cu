@@ -19,7 +19,9 @@
 #include "render_common.cuh"
 
 #ifndef RN_FWD_MINB
-#define RN_FWD_MINB 14  // minimum resident blocks per SM asked of ptxas (register budget)
+#define RN_FWD_MINB 12  // minimum resident blocks per SM asked of ptxas (register budget): 72 registers, 14 blocks resident.
+                        // Measured: 10 -> 80 registers, 12 blocks: equal; 16 -> 64 registers, 16 blocks: 10 % SLOWER
+                        // (shared memory grows with the blocks and comes out of the L1 the gathers live on)
 #endif
 
 namespace {
