@@ -1,8 +1,13 @@
 """include/mg.h: "Calls may overlap on different streams, and be issued from different host threads, as long as they share
 no output or scratch buffer: the library keeps no device-side state of its own".  Two host threads, each with its own
 stream, frame buffers and scene, run the whole hot path repeatedly at the same time; every result must be what the same
-frame gives when it runs alone -- bit for bit for the integers, the image and final_T (deterministic), and within the
-reordering of float atomics for the gradients."""
+frame gives when it runs alone -- bit for bit for the integers, the image and final_T (deterministic).  The gradients are
+not deterministic even for one frame alone: render_bwd sums with float atomics, whose order changes from run to run (a
+few ulp on each sum), and mg_preprocess_bwd amplifies that through the conic -> covariance map of elongated splats (the
+chain that needs fp64).  They are held to the bounds the parity tests hold them to against the oracle
+(1e-3 relative per element with a floor of 1e-4 of the array's largest element, and a relative 2-norm of 1e-4 per
+array: two solo runs of the 60 k-Gaussian outdoor scene already differ by 3e-6 .. 1.4e-5 in dL/dlog_scales); the difference between TWO SOLO runs of the same frame is printed beside the concurrent one as the noise floor.
+A library with shared device state gives a wrong R or other lists, not ulp noise."""
 import threading
 
 import numpy as np
@@ -42,6 +47,7 @@ def test_two_frames_on_two_streams_from_two_threads():
     specs = [lambda: scenes.config2(), lambda: scenes.config3(n=60_000, width=333, height=211)]
     scs = [f() for f in specs]
     alone = [_run_alone(sc) for sc in scs]
+    alone2 = [_run_alone(sc) for sc in scs]  # the noise floor of the float atomics
     results, errors = [None, None], []
     start = threading.Barrier(2)
 
@@ -76,7 +82,14 @@ def test_two_frames_on_two_streams_from_two_threads():
         assert got["R"] == ref["R"]
         for name in EXACT + ["sorted_ids"]:
             assert torch.equal(got[name], ref[name]), (k, name)
+        for name in EXACT + ["sorted_ids"]:
+            assert torch.equal(alone2[k][name], ref[name]), (k, name, "not deterministic alone")
         for name in GRADS:
-            a, b = got[name].double(), ref[name].double()
-            scale = float(b.abs().max())
-            assert float((a - b).abs().max()) <= 2e-5 * scale + 1e-30, (k, name)
+            a, b, b2 = got[name].double(), ref[name].double(), alone2[k][name].double()
+            scale, nrm = float(b.abs().max()), float(b.norm())
+            err, floor = (a - b).abs(), (b2 - b).abs()
+            print("CONCURRENCY", k, name, "rel 2-norm concurrent %.2e, solo vs solo %.2e; max|d| / max|ref| %.2e, solo %.2e"
+                  % (float((a - b).norm()) / max(nrm, 1e-300), float((b2 - b).norm()) / max(nrm, 1e-300),
+                     float(err.max()) / max(scale, 1e-300), float(floor.max()) / max(scale, 1e-300)))
+            assert float((a - b).norm()) <= 1e-4 * nrm + 1e-30, (k, name)  # parity_util.L2_CLEAN
+            assert bool((err <= 1e-3 * b.abs() + 1e-4 * scale + 1e-30).all()), (k, name)
