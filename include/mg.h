@@ -20,7 +20,8 @@
  *     asynchronous.
  *     Calls may overlap on different streams, and be issued from different host threads, as long as they
  *     share no output or scratch buffer: the library keeps no device-side state of its own (every counter
- *     lives in caller memory) and its per-device one-time initialisations are thread-safe.
+ *     lives in caller memory) and its per-device one-time initialisations are thread-safe.  The one exception
+ *     is mg_render_loss_static, whose scratch is an array inside the library: see there.
  *   - Domain: finite inputs; quats need not be unit but |q|^2 must be a normal fp32 number (1e-19 < |q| < 1e19) --
  *     a zero quaternion has no rotation, its covariance is not a number and the Gaussian is culled (radius 0, exact
  *     zeros everywhere), and a norm that under- or overflows in fp32 behaves the same; exp(log_scale) and the projected
@@ -197,6 +198,31 @@ int mg_compact(int64_t N, const uint8_t* keep, int32_t n_arrays, const float* co
 size_t mg_render_loss_workspace_bytes(int32_t width, int32_t height);
 int mg_render_loss(int32_t width, int32_t height, const float* image, const float* target, float lambda_dssim,
                    float* dL_dimage, double* stats, void* workspace, size_t workspace_bytes, void* stream);
+
+/* mg_render_loss_static: the same loss and gradient, for a caller that cannot provide a workspace because it cannot
+ * allocate device memory where it needs the loss -- code running inside an application whose own memory manager claimed
+ * the whole GPU at start-up and hands it only input and output buffers, a plug-in or callback bound to "no allocation
+ * after initialisation", a frame loop in which the device-wide synchronisation of cudaMalloc / cudaFree is not
+ * acceptable.  The call allocates and frees nothing, on the host side of CUDA or the device side: its scratch (9 floats
+ * per pixel) is an array built into the library's device image.
+ *   Limit: width * height <= MG_RENDER_LOSS_STATIC_MAX_PIXELS (2^21: 1920 x 1080 fits); a larger image is rejected with
+ *   MG_ERR_CAPACITY and a message that names the limit -- use mg_render_loss with your own workspace then.
+ *   Cost: 72 MiB of device memory (9 * 4 B * 2^21), reserved on EVERY GPU on which the CUDA runtime loads this library's
+ *   code (at the latest at the first render-loss call there) and held until the process exits, whether or not
+ *   mg_render_loss_static is ever called.
+ *   First call on a device: looks up the array's device address (cudaGetSymbolAddress, with that device current; the
+ *   result is cached per device) and uploads the filter window.  That makes the CUDA runtime load the kernels and reserve
+ *   the array, so make the first call on each device during set-up, outside any stream capture and before the point from
+ *   which nothing may be allocated.  Later calls only enqueue a 24-byte clear of `stats` and three kernels on `stream`.
+ *   Sharing: all calls on a device use the same array, and it keeps what the last call wrote.  Nothing in it needs to
+ *   start at zero (every element a call reads it has written itself), so calls of any image sizes may follow one another
+ *   on one stream.  Two calls that can run on the GPU at the same time (different streams, or different host threads
+ *   without ordering between their streams) RACE on it and give wrong gradients: order them, or give all but one of
+ *   them mg_render_loss with a workspace.
+ * image, target, dL_dimage, stats, lambda_dssim, the outputs and the error codes otherwise: exactly as mg_render_loss. */
+#define MG_RENDER_LOSS_STATIC_MAX_PIXELS (1 << 21)
+int mg_render_loss_static(int32_t width, int32_t height, const float* image, const float* target, float lambda_dssim,
+                          float* dL_dimage, double* stats, void* stream);
 
 /* ---- Density-control statistics and the optimiser step.  The paper keeps "the densification
  * scheme" and the training procedure of the 3DGS method it modifies and prints neither; DESIGN.md

@@ -35,7 +35,7 @@ class mg_camera(C.Structure):
 EXPORTS = ["mg_last_error_string", "mg_version", "mg_workspace_bytes", "mg_preprocess", "mg_bin_sort",
            "mg_render_fwd", "mg_render_bwd", "mg_preprocess_bwd", "mg_mask_sample", "mg_mask_sample_bwd", "mg_mask_loss",
            "mg_mask_prune_keep", "mg_compact_workspace_bytes", "mg_compact", "mg_render_loss_workspace_bytes",
-           "mg_render_loss", "mg_density_stats", "mg_adam_step", "mg_measure_fp32_peak", "mg_debug_set_lookback_spin_limit"]
+           "mg_render_loss", "mg_render_loss_static", "mg_density_stats", "mg_adam_step", "mg_measure_fp32_peak", "mg_debug_set_lookback_spin_limit"]
 
 
 def lib():
@@ -205,6 +205,18 @@ def mg_render_loss(image, target, lambda_dssim, dL_dimage, stats, workspace):
     _check(lib().mg_render_loss(C.c_int32(W), C.c_int32(H), _ptr(image, F32), _ptr(target, F32), C.c_float(lambda_dssim),
                                 _ptr(dL_dimage, F32), _ptr(stats, torch.float64), _ptr(workspace, U8),
                                 C.c_size_t(workspace.numel()), _stream()))
+
+
+RENDER_LOSS_STATIC_MAX_PIXELS = 1 << 21  # MG_RENDER_LOSS_STATIC_MAX_PIXELS of include/mg.h
+
+
+def mg_render_loss_static(image, target, lambda_dssim, dL_dimage, stats):
+    """mg_render_loss without a workspace argument, for callers that cannot allocate device memory: the scratch is an
+    array inside libmg.so (72 MiB per GPU), shared by all calls on a device -- calls that overlap on the GPU race.
+    Images of more than RENDER_LOSS_STATIC_MAX_PIXELS pixels raise MgError(MG_ERR_CAPACITY).  See include/mg.h."""
+    _, H, W = image.shape
+    _check(lib().mg_render_loss_static(C.c_int32(W), C.c_int32(H), _ptr(image, F32), _ptr(target, F32),
+                                       C.c_float(lambda_dssim), _ptr(dL_dimage, F32), _ptr(stats, torch.float64), _stream()))
 
 
 def mg_density_stats(dL_dmeans2d, radii, scale, grad_accum, denom, max_radii):

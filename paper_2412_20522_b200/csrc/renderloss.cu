@@ -236,3 +236,55 @@ extern "C" int mg_render_loss(int32_t width, int32_t height, const float* image,
   MG_CHECK_LAUNCH();
   return MG_OK;
 }
+
+// ---- mg_render_loss_static: mg_render_loss for callers that have no way to hand over a workspace.
+// Some hosts of this library may not allocate device memory at the point where they need the loss: a renderer or
+// trainer embedded in an application whose memory manager took all of the GPU's memory at start-up and hands out only
+// the input and output buffers; a plug-in or callback that runs under a "no allocation after initialisation" rule; a
+// per-frame loop that must not stall, where cudaMalloc / cudaFree would synchronise the whole device.  For them the
+// three derivative maps that the forward kernel leaves for the backward kernel (9 floats per pixel) live in this
+// file-scope array, which belongs to the library's image on the device: it is reserved on every GPU that loads this
+// part of the library and stays reserved until the process ends (72 MiB at the limit below).
+//
+// g_rl_scratch is a device symbol.  In host code its name is only a stand-in that the runtime maps to the device
+// address; it must never be passed to a kernel as it is.  The address is looked up once per device, with that device
+// current, by cudaGetSymbolAddress -- and that look-up is what makes the runtime load this file's kernels and
+// reserve the array on the device -- then cached.  After that the call is the existing path, given that address as
+// its workspace: the kernels and their arithmetic are the same.
+// Nothing in the array has to be zero when a call starts: every element the backward kernel reads (the pixels inside
+// the image) was written by the forward kernel of the same call, whatever an earlier call with another image size
+// left behind; the three sums are in the caller's `stats`, which the call clears itself.
+constexpr size_t RL_STATIC_FLOATS = 9 * (size_t)MG_RENDER_LOSS_STATIC_MAX_PIXELS;
+static __device__ __align__(256) float g_rl_scratch[RL_STATIC_FLOATS];
+
+extern "C" int mg_render_loss_static(int32_t width, int32_t height, const float* image, const float* target,
+                                     float lambda_dssim, float* dL_dimage, double* stats, void* stream) {
+  MG_REQUIRE(width > 0 && height > 0, "image size must be positive");
+  const unsigned long long pixels = (unsigned long long)width * (unsigned long long)height;
+  if (pixels > (unsigned long long)MG_RENDER_LOSS_STATIC_MAX_PIXELS) {
+    mg_set_error("mg_render_loss_static: a %d x %d image has %llu pixels, the built-in scratch holds at most %llu "
+                 "(MG_RENDER_LOSS_STATIC_MAX_PIXELS); use mg_render_loss with a workspace of your own",
+                 width, height, pixels, (unsigned long long)MG_RENDER_LOSS_STATIC_MAX_PIXELS);
+    return MG_ERR_CAPACITY;
+  }
+  static MgOncePerDevice looked_up;
+  static float* address_on[64];  // device address of g_rl_scratch, per device; written before looked_up is set
+  int dev = 0;
+  if (int rc = mg_current_device(&dev, nullptr)) return rc;
+  float* scratch = nullptr;
+  if (dev < 64 && looked_up.is_done(dev)) {
+    scratch = __atomic_load_n(&address_on[dev], __ATOMIC_RELAXED);
+  } else {
+    MG_CHECK_CUDA(cudaGetSymbolAddress((void**)&scratch, g_rl_scratch));
+    if (scratch == nullptr) {
+      mg_set_error("cudaGetSymbolAddress returned a null address for the built-in scratch");
+      return MG_ERR_CUDA;
+    }
+    if (dev < 64) {
+      __atomic_store_n(&address_on[dev], scratch, __ATOMIC_RELAXED);
+      looked_up.set_done(dev);
+    }
+  }
+  return mg_render_loss(width, height, image, target, lambda_dssim, dL_dimage, stats, scratch,
+                        RL_STATIC_FLOATS * sizeof(float), stream);
+}
