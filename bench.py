@@ -603,10 +603,22 @@ def main():
             if bound == "alu":
                 ach, peak, unit = work / sec / 1e12, fp32_peak, "TFLOP/s"
             else:
-                ach, peak, unit = work / sec / 1e9, hbm_gbs, "GB/s"
+                # An HBM-bound call is credited with the bytes it had to move AND did move: the per-Gaussian constants
+                # charge every row, but a kernel may skip rows that need no work (mg_preprocess_bwd does not touch the
+                # SH rows of Gaussians without a gradient), and bytes nobody read are not bandwidth.  `frac` therefore
+                # uses min(algorithmic, ncu DRAM traffic); both fractions are printed beside it.
+                moved = traffic.get(call)
+                charged = min(work, moved) if moved else work
+                ach, peak, unit = charged / sec / 1e9, hbm_gbs, "GB/s"
+                extra = {"charged_bytes": charged, "frac_algorithmic": work / sec / 1e9 / peak,
+                         "frac_moved": (moved / sec / 1e9 / peak) if moved else None}
+                if call == "bin_sort":  # the scheme's own byte count says nothing about the scheme: 4 B per key is any sort's floor
+                    extra["frac_of_4B_per_key_floor"] = wc["R"] * 4 / sec / 1e9 / peak
             rooflines[call] = {"bound": bound, "achieved": ach, "peak": peak, "unit": unit, "frac": ach / peak,
                                "traffic": traffic.get(call), "work_per_launch": work, "ms": per_call[call],
                                "share_of_step": per_call[call] / tot}
+            if bound != "alu":
+                rooflines[call].update(extra)
         dom = max(("render_fwd", "render_bwd"), key=lambda n: per_call[n])
         survey = wc[dom[7:] + "_pair_evals"] * FLOP_PAIR + wc[dom[7:] + "_blends"] * (FLOP_BLEND_BWD if dom == "render_bwd" else FLOP_BLEND_FWD)
         roofline = dict(rooflines[dom], kernel=dom + "_kernel",

@@ -195,8 +195,8 @@ def test_background_colour(oracle):
 @pytest.mark.parametrize("degree", [1, 2])
 def test_sh_degrees_1_and_2(oracle, degree):
     """The configs use SH degree 0 and 3 only; mg_preprocess / mg_preprocess_bwd have one kernel instance per degree, and
-    degree 1 (48-byte rows: bulk copies) and degree 2 (108-byte rows: not a multiple of 16, loads by flat position) take
-    different staging paths.  config 2's geometry, N ragged against a warp and a block, higher bands strong enough to
+    degree 1 (48-byte rows: float4 loads) and degree 2 (108-byte rows: not a multiple of 16, scalar loads by flat position)
+    take different staging paths.  config 2's geometry, N ragged against a warp and a block, higher bands strong enough to
     clamp channels; the whole path is run, projection and projection backward are compared (staged)."""
     import dataclasses
 
