@@ -35,30 +35,33 @@ class mg_camera(C.Structure):
 EXPORTS = ["mg_last_error_string", "mg_version", "mg_workspace_bytes", "mg_preprocess", "mg_bin_sort",
            "mg_render_fwd", "mg_render_bwd", "mg_preprocess_bwd", "mg_mask_sample", "mg_mask_sample_bwd", "mg_mask_loss",
            "mg_mask_prune_keep", "mg_compact_workspace_bytes", "mg_compact", "mg_render_loss_workspace_bytes",
-           "mg_render_loss", "mg_render_loss_static", "mg_density_stats", "mg_adam_step", "mg_measure_fp32_peak", "mg_debug_set_lookback_spin_limit"]
+           "mg_render_loss", "mg_render_loss_static", "mg_density_stats", "mg_adam_step", "mg_measure_fp32_peak"]
+
+
+def load_library(path):
+    """ctypes handle of a build of the library at `path`, with the return and argument types of include/mg.h set."""
+    if not os.path.exists(path):
+        raise MgError(MG_ERR_CUDA, f"{path} not built; run python -m paper_2412_20522_b200.build "
+                                   "(there is no CPU fallback)")
+    L = C.CDLL(path)
+    L.mg_last_error_string.restype = C.c_char_p
+    L.mg_workspace_bytes.restype = C.c_size_t
+    L.mg_workspace_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int32, C.c_uint64]
+    L.mg_render_loss_workspace_bytes.restype = C.c_size_t
+    L.mg_render_loss_workspace_bytes.argtypes = [C.c_int32, C.c_int32]
+    L.mg_compact_workspace_bytes.restype = C.c_size_t
+    L.mg_compact_workspace_bytes.argtypes = [C.c_int64]
+    for name in EXPORTS[3:]:
+        if not name.endswith("_workspace_bytes"):
+            getattr(L, name).restype = C.c_int
+    return L
 
 
 def lib():
     """Load libmg.so (built by `python -m paper_2412_20522_b200.build`).  Raises if it is missing."""
     global _lib
     if _lib is None:
-        if not os.path.exists(LIB_PATH):
-            raise MgError(MG_ERR_CUDA, f"{LIB_PATH} not built; run python -m paper_2412_20522_b200.build "
-                                       "(there is no CPU fallback)")
-        L = C.CDLL(LIB_PATH)
-        L.mg_last_error_string.restype = C.c_char_p
-        L.mg_workspace_bytes.restype = C.c_size_t
-        L.mg_workspace_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int32, C.c_uint64]
-        L.mg_render_loss_workspace_bytes.restype = C.c_size_t
-        L.mg_render_loss_workspace_bytes.argtypes = [C.c_int32, C.c_int32]
-        L.mg_compact_workspace_bytes.restype = C.c_size_t
-        L.mg_compact_workspace_bytes.argtypes = [C.c_int64]
-        L.mg_debug_set_lookback_spin_limit.restype = None
-        L.mg_debug_set_lookback_spin_limit.argtypes = [C.c_int]
-        for name in EXPORTS[3:]:
-            if not name.endswith("_workspace_bytes") and not name.startswith("mg_debug"):
-                getattr(L, name).restype = C.c_int
-        _lib = L
+        _lib = load_library(LIB_PATH)
     return _lib
 
 

@@ -117,7 +117,9 @@ __device__ __forceinline__ unsigned long long ld_relaxed_u64(const unsigned long
 constexpr unsigned long long LB_AGGREGATE = 1ull << 32;  // status word = flag << 32 | count
 constexpr unsigned long long LB_INCLUSIVE = 2ull << 32;
 constexpr int LB_SPIN_LIMIT = 1 << 26;                   // polls of one status word before a look-back gives up
+#ifdef MG_TESTING  // the test build only (libmg_testing.so): the shipped library has neither the hook nor its state
 std::atomic<int> g_spin_limit{LB_SPIN_LIMIT};             // mg_debug_set_lookback_spin_limit (failure injection in tests)
+#endif
 
 // One radix pass = ONE kernel (single-pass chained scan with decoupled look-back): a block takes the next
 // logical tile by ticket, ranks its 4096 keys, publishes its per-digit counts, and obtains its per-digit
@@ -493,10 +495,12 @@ __global__ void __launch_bounds__(32 * XP_MAX_WARPS) row_expand_kernel(
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t chunk = blockIdx.x * (uint32_t)warps_per_block + warp;
   if (chunk >= n_chunks) return;
-  // capacity overflow: only the counts are taken; a failed sort (overflow == 2) left `order` undefined: nothing is read
-  if (ctl->overflow && (!kCount || ctl->overflow == 2u)) return;
+  // capacity overflow: only the counts are taken.  A failed sort (overflow == 2) left `order` undefined: nothing of it is
+  // read and every count is written as zero, so that the scan and the plan that follow work on defined numbers.
+  const uint32_t ov = ctl->overflow;
+  if (ov && !kCount) return;
   uint32_t* cnt = xp_smem + (size_t)warp * (gh + 1);
-  const uint32_t nvis = ctl->nvis;
+  const uint32_t nvis = ov == 2u ? 0u : ctl->nvis;
   const uint32_t k0 = chunk * (uint32_t)XP_CHUNK;
   for (int b = lane; b <= gh; b += 32) cnt[b] = (kCount || b == gh) ? 0u : table_r[(size_t)b * n_chunks + chunk];
   __syncwarp();
@@ -744,7 +748,9 @@ extern "C" size_t mg_workspace_bytes(int64_t N, int32_t width, int32_t height, u
   return make_layout(N, gw, gh, R_capacity).total;
 }
 
+#ifdef MG_TESTING
 extern "C" void mg_debug_set_lookback_spin_limit(int polls) { g_spin_limit.store(polls < 0 ? LB_SPIN_LIMIT : polls); }
+#endif
 
 extern "C" int mg_bin_sort(const mg_camera* cam, int64_t N, const float* depths, const int32_t* rects,
                            const uint32_t* tiles_touched, uint64_t R_capacity, void* workspace, size_t workspace_bytes,
@@ -797,7 +803,11 @@ extern "C" int mg_bin_sort(const mg_camera* cam, int64_t N, const float* depths,
     attr_set.set_done(dev);
   }
   const int dk_grid = sms * 8;
+#ifdef MG_TESTING
   const int spin_limit = g_spin_limit.load(std::memory_order_relaxed);
+#else
+  const int spin_limit = LB_SPIN_LIMIT;
+#endif
   MG_CHECK_CUDA(cudaMemsetAsync(status, 0, sizeof(unsigned long long) * 4 * (size_t)L.nblk_sort * RS_BINS, st));
   {
     const int64_t want = (N + 255) / 256;

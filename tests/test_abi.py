@@ -17,9 +17,12 @@ def lib():
     return binding.lib()
 
 
-def declared_symbols():
+def declared_symbols(testing=False):
+    """Functions include/mg.h declares: the shipped ABI, or (testing=True) only what -DMG_TESTING adds to it."""
     text = open(os.path.join(ROOT, "include", "mg.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    guarded = re.findall(r"#ifdef MG_TESTING\n(.*?)#endif", text, flags=re.S)
+    text = "\n".join(guarded) if testing else re.sub(r"#ifdef MG_TESTING\n.*?#endif", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(mg_[a-z0-9_]+)\s*\(", text)))
 
 
@@ -36,6 +39,21 @@ def test_library_exports_every_declared_symbol(lib):
         assert hasattr(lib, s), f"libmg.so does not export {s}"
     assert sorted(binding.EXPORTS) == declared_symbols()
     assert lib.mg_version() >= 100
+
+
+def test_test_hooks_are_only_in_the_test_build(lib):
+    """mg_debug_set_lookback_spin_limit is process-wide state that can make every sort fail: it is compiled only with
+    -DMG_TESTING, into libmg_testing.so, and the shipped libmg.so must not export it."""
+    from paper_2412_20522_b200 import build
+
+    hooks = declared_symbols(testing=True)
+    assert hooks == ["mg_debug_set_lookback_spin_limit"]
+    testing = C.CDLL(build.LIB_TESTING)
+    for s in hooks:
+        assert not hasattr(lib, s), f"libmg.so exports the test hook {s}"
+        assert hasattr(testing, s), f"libmg_testing.so lacks {s}"
+    for s in declared_symbols():
+        assert hasattr(testing, s)
 
 
 def test_workspace_bytes_host_logic(lib):
