@@ -6,11 +6,16 @@
 //   mg_compact          stable compaction of the attribute arrays by the keep flags
 // All elementwise and HBM-bound: one pass over the data, coalesced, no intermediate arrays.  Random numbers are
 // inputs (uniforms in (0,1)); the library draws none.
+#include <cooperative_groups.h>
+
 #include "mg_common.cuh"
+
+namespace cg = cooperative_groups;
 
 namespace {
 
 constexpr int MH_THREADS = 256;
+constexpr int ML_BLOCKS_PER_SM = 4;  // mg_mask_loss: grid = at most this many blocks per SM (and never more than can be resident)
 
 // d = (s_1 + g_1) - (s_0 + g_0) with g = -log(-log u): the hard sample is d > 0, the soft one sigmoid(d / tau).
 // A uniform outside (0,1) is taken as the nearest fp32 value inside it (include/mg.h, reading 29): the noise
@@ -45,20 +50,23 @@ __global__ void __launch_bounds__(MH_THREADS) mask_sample_bwd_kernel(int64_t N, 
 
 // stats[0] += sum of masks (double: exact for 0/1 masks whatever the order of the atomics)
 // L_m and its gradient in ONE kernel (two launches in round 1).  Every element needs the mean over all of them, so the
-// grid meets once: phase 1 sums the masks into stats[0]; a barrier; phase 2 adds lambda_m 2 mean / N to dL_dmask.  The
-// barrier is two counters kept in stats[1] and stats[2] (outputs that nobody reads before the end): blocks arrive, spin
-// until all have arrived, do phase 2, and leave; the block that leaves last overwrites the counters with the results,
-// when no block can be looking at them any more.  All blocks must be resident at once for the spin to end: the grid is
-// sized to that and the launch is cooperative, so the runtime refuses a grid that would not be.
+// grid meets once: phase 1 sums the masks into stats[0]; grid.sync(); phase 2 adds lambda_m 2 mean / N to dL_dmask and
+// block 0 writes the two results.  The barrier is the cooperative-groups one (the launch is cooperative, so the runtime
+// refuses a grid that could not be resident at once); it keeps its state outside the caller's arrays.  The grid is a few
+// blocks per SM, not the whole GPU: a 12 MB read needs no more, and the rest of the GPU stays free for work on other
+// streams.  Both phases move float4s (masks and dL_dmask are 16-byte aligned, include/mg.h), the tail singly.
 __global__ void __launch_bounds__(MH_THREADS) mask_loss_kernel(int64_t N, const float* __restrict__ masks, double lambda_m,
                                                                float* __restrict__ dL_dmask, double* __restrict__ stats) {
   __shared__ double part[MH_THREADS / 32];
-  __shared__ double s_total;
-  unsigned long long* arrive = reinterpret_cast<unsigned long long*>(&stats[1]);
-  unsigned long long* leave = reinterpret_cast<unsigned long long*>(&stats[2]);
   const int64_t stride = (int64_t)gridDim.x * MH_THREADS, first = (int64_t)blockIdx.x * MH_THREADS + threadIdx.x;
+  const int64_t n4 = N >> 2;
+  const float4* __restrict__ masks4 = reinterpret_cast<const float4*>(masks);
   double s = 0.0;
-  for (int64_t i = first; i < N; i += stride) s += (double)masks[i];
+  for (int64_t i = first; i < n4; i += stride) {
+    const float4 v = masks4[i];
+    s += ((double)v.x + (double)v.y) + ((double)v.z + (double)v.w);
+  }
+  for (int64_t i = 4 * n4 + first; i < N; i += stride) s += (double)masks[i];
 #pragma unroll
   for (int o = 16; o >= 1; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
   if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = s;
@@ -68,21 +76,21 @@ __global__ void __launch_bounds__(MH_THREADS) mask_loss_kernel(int64_t N, const 
 #pragma unroll
     for (int w = 0; w < MH_THREADS / 32; w++) t += part[w];
     if (t != 0.0) atomicAdd(&stats[0], t);
-    __threadfence();
-    atomicAdd(arrive, 1ull);
-    while (*reinterpret_cast<volatile unsigned long long*>(arrive) < (unsigned long long)gridDim.x) {}
-    __threadfence();
-    s_total = *reinterpret_cast<volatile double*>(&stats[0]);
   }
-  __syncthreads();
-  const double mean = s_total / (double)N;
+  cg::this_grid().sync();
+  const double mean = *reinterpret_cast<volatile double*>(&stats[0]) / (double)N;
   if (dL_dmask) {
     const float add = (float)(lambda_m * 2.0 * mean / (double)N);
-    for (int64_t i = first; i < N; i += stride) dL_dmask[i] += add;
+    float4* __restrict__ g4 = reinterpret_cast<float4*>(dL_dmask);
+    for (int64_t i = first; i < n4; i += stride) {
+      float4 v = g4[i];
+      v.x += add; v.y += add; v.z += add; v.w += add;
+      g4[i] = v;
+    }
+    for (int64_t i = 4 * n4 + first; i < N; i += stride) dL_dmask[i] += add;
   }
-  __syncthreads();
-  if (threadIdx.x == 0 && atomicAdd(leave, 1ull) == (unsigned long long)gridDim.x - 1) {
-    stats[1] = lambda_m * mean * mean;  // every block has left the spin: the counters are free
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    stats[1] = lambda_m * mean * mean;
     stats[2] = mean;
   }
 }
@@ -216,11 +224,22 @@ extern "C" int mg_mask_loss(int64_t N, const float* masks, float lambda_m, float
   MG_REQUIRE(masks && stats, "null array");
   cudaStream_t st = (cudaStream_t)stream;
   MG_CHECK_CUDA(cudaMemsetAsync(stats, 0, 3 * sizeof(double), st));
-  const int64_t want = (N + MH_THREADS - 1) / MH_THREADS;
-  int sms = 0, per_sm = 0;
-  if (int rc = mg_current_device(nullptr, &sms)) return rc;
-  MG_CHECK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mask_loss_kernel, MH_THREADS, 0));
-  const int64_t resident = (int64_t)sms * (per_sm > 0 ? per_sm : 1);
+  const int64_t want = (N / 4 + MH_THREADS - 1) / MH_THREADS + 1;
+  static MgOncePerDevice asked;   // the occupancy query costs as much host time as the kernel runs: once per device
+  static int per_sm_of[64];
+  int dev = 0, sms = 0, per_sm = 0;
+  if (int rc = mg_current_device(&dev, &sms)) return rc;
+  if (dev < 64 && asked.is_done(dev)) {
+    per_sm = __atomic_load_n(&per_sm_of[dev], __ATOMIC_RELAXED);
+  } else {
+    MG_CHECK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mask_loss_kernel, MH_THREADS, 0));
+    if (per_sm < 1) per_sm = 1;
+    if (dev < 64) {
+      __atomic_store_n(&per_sm_of[dev], per_sm, __ATOMIC_RELAXED);
+      asked.set_done(dev);
+    }
+  }
+  const int64_t resident = (int64_t)sms * (per_sm < ML_BLOCKS_PER_SM ? per_sm : ML_BLOCKS_PER_SM);
   const unsigned grid = (unsigned)(want < resident ? want : resident);
   double lam = (double)lambda_m;
   void* args[] = {(void*)&N, (void*)&masks, (void*)&lam, (void*)&dL_dmask, (void*)&stats};
