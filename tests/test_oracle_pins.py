@@ -420,7 +420,7 @@ def test_projection_matches_numpy_ewa(oracle):
     gw, gh = 16, 16
     R, t = np.asarray(cam.R, np.float32).astype(np.float64), np.asarray(cam.t, np.float32).astype(np.float64)
     fx, fy, cx, cy = (float(np.float32(v)) for v in (cam.fx, cam.fy, cam.cx, cam.cy))
-    nvis = 0
+    nvis, margins = 0, []
     for i in range(0, sc.N, 7):
         p = sc.means[i].astype(np.float64)
         tc = R @ p + t
@@ -457,7 +457,19 @@ def test_projection_matches_numpy_ewa(oracle):
         np.testing.assert_allclose(pre["depths"][i], tc[2], rtol=1e-14)
         assert pre["radii"][i] == rad
         assert pre["rects"][i].tolist() == [x0, y0, x1, y1] and pre["tiles_touched"][i] == (x1 - x0) * (y1 - y0)
+        # `margin` (gates which Gaussians the GPU comparison may exempt from bit-exact integers): how far, in pixels /
+        # depth units, the nearest of this Gaussian's integer decisions is from flipping -- the near-plane test, the
+        # ceil of the radius, the four floors of the tile rectangle (a quotient in tiles is 16 pixels per unit).
+        to_int = lambda v: abs(v - np.rint(v))
+        quot = [(m2[0] - rad) / 16, (m2[0] + rad + 15) / 16, (m2[1] - rad) / 16, (m2[1] + rad + 15) / 16]
+        want = min(abs(tc[2] - 0.2), to_int(3 * np.sqrt(lam_f)), 16 * min(to_int(q) for q in quot))
+        np.testing.assert_allclose(pre["margin"][i], want, rtol=1e-6, atol=1e-9)
+        margins.append(want)
     assert nvis > 200
+    # the pin bites: margins spread over the whole range a distance to the nearest integer can take, and moving an input
+    # by less than a Gaussian's margin leaves its integers alone while the smallest margins sit near a flip
+    margins = np.array(margins)
+    assert margins.min() < 0.02 and margins.max() > 0.3 and (margins <= 0.5 + 1e-12).all()
 
 
 # ---------------------------------------------------------------- tile shift (pixel-centre convention, reading 15)
