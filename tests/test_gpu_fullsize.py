@@ -1,8 +1,9 @@
 """Parity at BASELINE.json's full sizes -- configs[2] (3 M Gaussians, 1297x840: the bench workload), configs[3]
 (2.8 M, 1264x832, indoor) and configs[4] (6 M, 1920x1080, keep-probability 0.9: the largest size and the
-longest tile lists), camera 0, SH degree 3 -- in the launch configuration bench.py times.  Projection, sort and projection-backward are compared in full; the two
-blend kernels on a seeded sample of tiles the oracle can walk in seconds (the other tiles' ranges are
-emptied for both sides, which leaves the sampled tiles' arithmetic untouched)."""
+longest tile lists), camera 0, SH degree 3 -- in the launch configuration bench.py times.  Projection, sort, projection-backward AND the two
+blend kernels are compared in full at camera 0 (the oracle walks a whole frame in seconds on the box's cores); the three
+other cameras of config 5 compare the blend kernels on a seeded sample of tiles (the other tiles' ranges are emptied for
+both sides, which leaves the sampled tiles' arithmetic untouched)."""
 import numpy as np
 import pytest
 import torch
@@ -32,33 +33,28 @@ def test_full_size_projection_and_sort(full, oracle):
     print("PARITY", sc.name, "full size", dict(R=fr.R, preprocess=s1))
 
 
-def test_full_size_blend_on_sampled_tiles(full, oracle):
+# Whole-frame budgets: the largest fraction of pixels (forward) / Gaussians (backward) the staged comparison may set
+# aside as threshold-sensitive -- at most twice the counts observed on the B200 (profiles/r03_parity_counts.md).
+# Observed: pixels 0.00142 / 0.00168 / 0.00097, Gaussians 0.0440 / 0.0773 / 0.0142.
+WHOLE_FRAME_BUDGET = {"cfg3_outdoor": (0.0028, 0.088), "cfg4_indoor": (0.0033, 0.15), "cfg5_stress": (0.0019, 0.028)}
+
+
+def test_full_size_blend_whole_frame(full, oracle):
+    """north_star's target sentence, on every pixel: the masked forward and backward blend of the whole frame (all
+    4 346 / 4 108 / 8 160 tiles, in the launch configuration bench.py times: tile_order hint, full grid, the atomics'
+    contention of a whole frame) against the oracle's plain per-pixel walk over the same lists (staged: the oracle blends
+    the GPU's fp32 splats).  Image and final_T elementwise at 1e-5 + 1e-4, n_contrib bit-exact off the margin, the five
+    gradient arrays elementwise at 1e-3 on every Gaussian that no near-threshold decision touches, 2-norms on all."""
     sc, fr, g, m, gimg = full
     cam = sc.camera
-    gw, gh = mg.grid(cam)
-    rng = np.random.default_rng(12)
-    lens = (pu.u32(fr.tile_ranges)[:, 1] - pu.u32(fr.tile_ranges)[:, 0]).astype(np.int64)
-    tiles = set(rng.choice(gw * gh, 40, replace=False).tolist())
-    tiles |= {int(np.argmax(lens)), gw - 1, gw * gh - 1, gw * (gh - 1)}  # longest list + ragged corners
-    tiles = sorted(tiles)
-    ranges_full = pu.u32(fr.tile_ranges).copy()
-    ranges_s = np.zeros_like(ranges_full)
-    ranges_s[tiles] = ranges_full[tiles]
     ids = pu.u32(fr.sorted_ids)[: fr.R]
-    ref, s3 = pu.check_render_fwd(fr, cam, sc.masks, ids, ranges_s, tiles=tiles, max_flag_frac=4e-3)
-    print("PARITY", sc.name, "full size fwd sampled tiles", dict(tiles=len(tiles), render_fwd=s3))
-    # backward restricted to the same tiles on both sides
-    keep_ranges = fr.tile_ranges.clone()
-    fr.tile_ranges.copy_(torch.from_numpy(ranges_s.view(np.int32)).cuda())
-    fr.render_bwd(m, gimg)
-    torch.cuda.synchronize()
-    try:
-        _, s4 = pu.check_render_bwd(fr, cam, sc.N, sc.masks, ids, ranges_s, sc.dL_dimage(), max_flag_frac=2e-3)
-        print("PARITY", sc.name, "full size bwd sampled tiles", dict(render_bwd=s4))
-    finally:
-        fr.tile_ranges.copy_(keep_ranges)
-        fr.render_bwd(m, gimg)
-        torch.cuda.synchronize()
+    ranges = pu.u32(fr.tile_ranges).copy()
+    fwd_budget, bwd_budget = WHOLE_FRAME_BUDGET[sc.name]
+    _, s3 = pu.check_render_fwd(fr, cam, sc.masks, ids, ranges, max_flag_frac=fwd_budget)
+    assert s3["n_contrib_diff"] <= s3["n_flagged"]
+    print("PARITY", sc.name, "full size fwd whole frame", dict(tiles=int(ranges.shape[0]), render_fwd=s3))
+    _, s4 = pu.check_render_bwd(fr, cam, sc.N, sc.masks, ids, ranges, sc.dL_dimage(), max_flag_frac=bwd_budget)
+    print("PARITY", sc.name, "full size bwd whole frame", dict(render_bwd=s4))
 
 
 @pytest.mark.parametrize("cam_index", [5, 10, 15])
