@@ -23,19 +23,23 @@ def _need_gpu():
     mg.lib()  # fails loudly if libmg.so is missing: there is no fallback
 
 
-# Largest fraction of Gaussians the end-to-end gradient comparison may exempt as threshold-sensitive (about twice the
-# count observed on the B200, profiles/r02_parity_counts.md).
+# Largest fraction of Gaussians the end-to-end gradient comparison may exempt as threshold-sensitive (at most twice the
+# count observed on the B200, profiles/r03_parity_counts.md; cfg2: 0.375 observed).
 # End to end the fp32 chain (projection -> blend -> two backward stages) is held against the fp64 chain from the raw
-# inputs: the rounding of two stages compounds, so the elementwise bound is twice north_star's 1e-3 (which the staged
-# comparison of each call holds on its own) and the absolute floor is 1e-4 of the array's largest element.
-E2E_GRAD_RTOL = 2e-3
-E2E_GRAD_BUDGET = {"tiny": 0.0, "cfg1": 0.14, "cfg2": 0.5, "cfg3_small": 0.08, "cfg4_small": 0.07}
+# inputs at north_star's 1e-3 relative, elementwise, with the absolute floor of the staged projection-backward comparison
+# (1e-4 of the array's largest element: an element that is the sum of cancelling per-pixel terms has no relative accuracy
+# of its own).  Measured on the B200 at this tolerance: worst error / tolerance 0.24 (cfg4_small dL_dmeans2d), 0.235 (cfg2
+# dL_dquats), <= 0.16 everywhere else.  (With a floor of 1e-5 every array of every scene still passes except ONE element
+# each of cfg2 dL_dquats, at 1.09 x, and cfg4_small dL_dmeans2d, at 1.03 x.)
+E2E_GRAD_RTOL = 1e-3
+E2E_GRAD_FLOOR = 1e-4
+E2E_GRAD_BUDGET = {"tiny": 0.0, "cfg1": 0.136, "cfg2": 0.40, "cfg3_small": 0.072, "cfg4_small": 0.064}
 # Scenes whose END-TO-END comparison is ill-posed in fp32 and is therefore held in the 2-norm only.  "needles": the conic
 # that mg_preprocess stores is fp32 (relative rounding 6e-8 per component); at a pixel thousands of pixels from the
 # centre of a long thin splat the terms A dx^2, B dx dy, C dy^2 reach 1e4..1e6 and cancel, so that rounding alone moves
 # the exponent by 1e-3..1e-1 whatever the blend kernel does.  The kernel's own arithmetic on those splats is checked by
 # the STAGED test (the oracle runs on the fp32 conics), elementwise, with no allowance.
-E2E_L2_ONLY = {"needles": 3e-2}
+E2E_L2_ONLY = {"needles": 5e-3}  # observed 2.2e-3
 
 
 def small_scenes():
@@ -119,11 +123,14 @@ def test_end_to_end_gradient_parity(run, oracle):
     # blended behind it at those pixels) see one entry more or less.  Scenes with such Gaussians are compared in the
     # 2-norm only; the others elementwise on the non-flagged Gaussians.
     order_same = fr.R == len(ids) and np.array_equal(pu.u32(fr.sorted_ids)[: fr.R], ids)
+    # On every scene of this module the fp32 and the fp64 chain produce the same lists (observed on the B200); were that
+    # to change, the elementwise branch below would silently stop running -- so it is asserted, not assumed.
+    assert order_same and not unstable.any(), f"{name}: fp32 and fp64 lists differ (unstable={int(unstable.sum())})"
     clean = (rb["sens"] == 0) & ~unstable
     ref = {k: v for k, v in list(rb.items()) + list(pb.items()) if k.startswith("dL_")}
     if order_same and name not in E2E_L2_ONLY:
         out = pu.grads_vs_ref(fr, ref, list(ref), clean, max_flag_frac=E2E_GRAD_BUDGET[name], l2_clean=2e-4,
-                              rtol=E2E_GRAD_RTOL, floor_frac=1e-4)
+                              rtol=E2E_GRAD_RTOL, floor_frac=E2E_GRAD_FLOOR)
     else:
         out = {}
         for k, r in ref.items():
@@ -248,18 +255,32 @@ def test_projection_backward_with_dense_upstream_gradients(oracle):
     print("dense upstream", s5)
 
 
-def test_lookback_failure_is_reported_not_returned_as_an_order():
+def test_lookback_failure_is_reported_not_returned_as_an_order(monkeypatch):
     """include/mg.h, mg_bin_sort "Internal failure": a look-back that gives up must not yield a wrong order.  Injected
-    through the test hook: every look-back gives up at once."""
+    through the hook of the TEST build of the library (libmg_testing.so, -DMG_TESTING; the shipped libmg.so has no such
+    hook): every look-back gives up at once.  The first radix tile of a pass has no predecessor and never looks back, so
+    the scene must span several tiles for the injection to reach anything."""
+    import ctypes as C
+    import os
+
+    from paper_2412_20522_b200 import build
+
     sc = scenes.config2()
+    assert sc.N > 8 * 4096  # a radix tile is 4096 keys (RS_THREADS * RS_ITEMS of binsort.cu): at least 8 look-backs per pass
     g, m = mg.upload(sc)
     fr = mg.Frame(sc.camera, sc.N)
     fr.forward(g, m)
     torch.cuda.synchronize()
     R = fr.R
-    good = fr.tile_ranges.clone()
+    good, good_ids = fr.tile_ranges.clone(), fr.sorted_ids.clone()
+    assert os.path.exists(build.LIB_TESTING), "libmg_testing.so not built (python -m paper_2412_20522_b200.build)"
+    tl = mg.load_library(build.LIB_TESTING)
+    tl.mg_debug_set_lookback_spin_limit.restype = None
+    tl.mg_debug_set_lookback_spin_limit.argtypes = [C.c_int]
+    assert not hasattr(mg.lib(), "mg_debug_set_lookback_spin_limit")
+    monkeypatch.setattr(mg, "_lib", tl)  # from here on the binding's calls go through the test build
     try:
-        mg.lib().mg_debug_set_lookback_spin_limit(0)
+        tl.mg_debug_set_lookback_spin_limit(0)
         fr.sorted_ids.fill_(-1)
         fr.bin_sort()
         torch.cuda.synchronize()
@@ -269,10 +290,10 @@ def test_lookback_failure_is_reported_not_returned_as_an_order():
         torch.cuda.synchronize()
         assert (fr.n_contrib == 0).all()
     finally:
-        mg.lib().mg_debug_set_lookback_spin_limit(-1)
-    fr.bin_sort()
+        tl.mg_debug_set_lookback_spin_limit(-1)
+    fr.bin_sort()  # the test build without the injection: the same result as the shipped library
     torch.cuda.synchronize()
-    assert int(fr.R_host[1]) == R and torch.equal(fr.tile_ranges, good)
+    assert int(fr.R_host[1]) == R and torch.equal(fr.tile_ranges, good) and torch.equal(fr.sorted_ids[:R], good_ids[:R])
 
 
 # ------------------------------------------------------------------ edge cases
