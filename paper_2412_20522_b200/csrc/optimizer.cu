@@ -101,11 +101,15 @@ __global__ void __launch_bounds__(OP_THREADS) adam_kernel(const __grid_constant_
       adam_one(pn.y, g[k].y, mn.y, vn.y, P, step_size);
       adam_one(pn.z, g[k].z, mn.z, vn.z, P, step_size);
       adam_one(pn.w, g[k].w, mn.w, vn.w, P, step_size);
-      if (kRows && vis[k] != 0xfu) {  // the vector straddles a row that is not updated
-        if (!(vis[k] & 1u)) { pn.x = p[k].x; mn.x = m[k].x; vn.x = v[k].x; }
-        if (!(vis[k] & 2u)) { pn.y = p[k].y; mn.y = m[k].y; vn.y = v[k].y; }
-        if (!(vis[k] & 4u)) { pn.z = p[k].z; mn.z = m[k].z; vn.z = v[k].z; }
-        if (!(vis[k] & 8u)) { pn.w = p[k].w; mn.w = m[k].w; vn.w = v[k].w; }
+      if (kRows && vis[k] != 0xfu) {  // the vector straddles a row that is not updated: only the updated floats are
+        const float pa[4] = {pn.x, pn.y, pn.z, pn.w}, ma[4] = {mn.x, mn.y, mn.z, mn.w}, va[4] = {vn.x, vn.y, vn.z, vn.w};
+#pragma unroll
+        for (unsigned int j = 0; j < 4; j++) {  // stored, so that a skipped row is really not written (include/mg.h)
+          if ((vis[k] >> j) & 1u) {
+            G.p[e[k] + j] = pa[j]; G.m[e[k] + j] = ma[j]; G.v[e[k] + j] = va[j];
+          }
+        }
+        continue;
       }
       *reinterpret_cast<float4*>(G.p + e[k]) = pn;
       *reinterpret_cast<float4*>(G.m + e[k]) = mn;

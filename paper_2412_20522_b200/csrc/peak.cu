@@ -54,9 +54,16 @@ extern "C" int mg_measure_fp32_peak(double min_seconds, double* tflops_host, flo
   int sms = 0;
   if (int rc = mg_current_device(nullptr, &sms)) return rc;
   cudaStream_t st = (cudaStream_t)stream;
-  cudaEvent_t e0, e1;
-  MG_CHECK_CUDA(cudaEventCreate(&e0));
-  MG_CHECK_CUDA(cudaEventCreate(&e1));
+  struct Events {  // destroyed on every way out, the MG_CHECK_CUDA early returns included
+    cudaEvent_t a = nullptr, b = nullptr;
+    ~Events() {
+      if (a) cudaEventDestroy(a);
+      if (b) cudaEventDestroy(b);
+    }
+  } ev;
+  MG_CHECK_CUDA(cudaEventCreate(&ev.a));
+  MG_CHECK_CUDA(cudaEventCreate(&ev.b));
+  const cudaEvent_t e0 = ev.a, e1 = ev.b;
   const int grid = sms * 4;  // 4 blocks of 512 threads per SM: every warp slot taken
   const int iters = 256;
   for (int form = 0; form < 2; form++) {
@@ -85,7 +92,5 @@ extern "C" int mg_measure_fp32_peak(double min_seconds, double* tflops_host, flo
     tflops_host[2 * form] = flop / spent / 1e12;  // sustained over the whole measurement
     tflops_host[2 * form + 1] = best;             // best round (burst)
   }
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
   return MG_OK;
 }

@@ -68,6 +68,16 @@ def test_adam_step_parity_all_groups_one_launch(n, step):
     _check(groups, got, 0.9, 0.999, 1e-15, step)
 
 
+def test_adam_step_parity_at_the_bench_size():
+    """The size bench.py times (next_rows.optimizer): 3 M Gaussians, all attribute groups in one launch, 59 floats per
+    Gaussian = 177 M parameters -- block indices past 2^16 per group, element offsets past 2^27."""
+    n = 3_000_000
+    rng = np.random.default_rng(33)
+    groups = _groups(rng, n)
+    got = _run(groups, 0.9, 0.999, 1e-15, 7)
+    _check(groups, got, 0.9, 0.999, 1e-15, 7)
+
+
 def test_adam_first_step_from_zero_moments_is_a_sign_step():
     rng = np.random.default_rng(0)
     g = rng.normal(0, 1, (1000, 3)).astype(np.float32)
@@ -101,7 +111,7 @@ def test_adam_empty_and_argument_checks():
                         0.9, 0.999, 1e-15, 1, radii=torch.ones(8, dtype=torch.int32, device="cuda"))
 
 
-@pytest.mark.parametrize("n", [0, 1, 777, 300_000])
+@pytest.mark.parametrize("n", [0, 1, 777, 300_000, 3_000_000])
 def test_density_stats_parity(n):
     from oracle import optimizer as opt
 
