@@ -39,7 +39,7 @@ BYTES_PRE = (301, 109)     # mg_preprocess, per visible / per culled Gaussian
 BYTES_PRE_BWD = (513, 240)  # mg_preprocess_bwd, per visible / per culled Gaussian
 BYTES_SORT_KEY = 22        # mg_bin_sort, per duplicated key, this scheme; the floor of any scheme is 4
 # dram__bytes_read.sum + dram__bytes_write.sum per launch, summed over the kernels of each call: written by
-# `python -m paper_2412_20522_b200.ncu_summary` from the `ncu --set full` capture named in profiles/r02_final.md (section 3)
+# `python ncu_summary.py` from the `ncu --set full` capture named in profiles/r02_final.md (section 3)
 TRAFFIC_JSON = os.path.join(ROOT, "profiles", "r02_traffic.json")
 # kernels of libmg launched per step (memsets and copies not counted), see binsort.cu for the sort's list
 KERNELS_PER_STEP = {"preprocess": 1, "bin_sort": 2 + 4 + 5 + 6, "render_fwd": 1, "render_bwd": 1,
@@ -368,6 +368,67 @@ def bench_optimizer(sc, g, fr, hbm_gbs, reps=10):
     return out
 
 
+def bench_training_iteration(sc, g, fr, reps=10):
+    """One whole training iteration on the bench workload, the eleven C-ABI calls of DESIGN.md section 11 back to back
+    on one stream: mask_sample, preprocess, bin_sort, render_fwd, render_loss, render_bwd, mask_loss, mask_sample_bwd,
+    preprocess_bwd, density_stats, adam_step (all 59 floats per Gaussian + the 2 mask scores).  Parameters do change from
+    iteration to iteration (lr 1e-5: the scene stays the bench scene to within the noise of a few steps); the uniforms
+    are one fixed draw.  The sum of the rows timed one by one is printed beside it for comparison."""
+    import torch
+
+    from paper_2412_20522_b200 import binding as mg
+
+    n, cam = sc.N, sc.camera
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(7)
+    uniforms = torch.rand(n, 2, device="cuda", generator=gen).clamp_(1e-7, 1 - 1e-7)
+    scores = torch.zeros(n, 2, device="cuda")
+    scores[:, 1] = torch.randn(n, device="cuda", generator=gen)
+    names = ("means", "log_scales", "quats", "opacity_logits", "sh")
+    params = {k: g[k].clone() for k in names}
+    masks, soft = torch.empty(n, device="cuda"), torch.empty(n, device="cuda")
+    dL_dscores = torch.empty(n, 2, device="cuda")
+    fr.forward(params, torch.ones(n, device="cuda"))
+    fr.reserve(int(fr.R * 1.1))
+    target = fr.image.clone()
+    dL_dimage = torch.empty_like(fr.image)
+    lstats, mstats = (torch.zeros(3, dtype=torch.float64, device="cuda") for _ in range(2))
+    ws = torch.empty(mg.mg_render_loss_workspace_bytes(cam.width, cam.height), dtype=torch.uint8, device="cuda")
+    acc, den, mxr = (torch.zeros(n, device="cuda") for _ in range(3))
+    grads = dict(means=fr.dL_dmeans, log_scales=fr.dL_dlog_scales, quats=fr.dL_dquats, opacity_logits=fr.dL_dopacity_logits,
+                 sh=fr.dL_dsh)
+    groups = [(params[k], grads[k], torch.zeros_like(params[k]), torch.zeros_like(params[k]), 1e-5) for k in names]
+    groups.append((scores, dL_dscores, torch.zeros_like(scores), torch.zeros_like(scores), 1e-5))
+    it = [0]
+
+    def iteration():
+        it[0] += 1
+        mg.mg_mask_sample(scores, uniforms, 1.0, masks, soft)
+        fr.preprocess(params)  # no host sync inside the iteration: the sort buffers keep a 10 % reserve (below)
+        fr.bin_sort()
+        fr.render_fwd(masks)
+        mg.mg_render_loss(fr.image, target, 0.2, dL_dimage, lstats, ws)
+        fr.render_bwd(masks, dL_dimage)
+        fr.preprocess_bwd(params)
+        mg.mg_mask_loss(masks, 5e-4, fr.dL_dmask, mstats)
+        mg.mg_mask_sample_bwd(soft, fr.dL_dmask, 1.0, dL_dscores)
+        mg.mg_density_stats(fr.dL_dmeans2d, fr.radii, (cam.width / 2, cam.height / 2), acc, den, mxr)
+        mg.mg_adam_step(groups, 0.9, 0.999, 1e-15, it[0])
+
+    for _ in range(3):
+        iteration()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(reps):
+        iteration()
+    e1.record()
+    torch.cuda.synchronize()
+    assert int(fr.R_host[1]) <= fr.R_capacity, "R outgrew the reserve during the timed iterations"
+    return {"ms": round(e0.elapsed_time(e1) / reps, 4), "calls": 11, "iterations_timed": reps,
+            "loss_render": float(lstats[2]), "mean_mask": float(mstats[2])}
+
+
 def n_threads():
     try:
         return len(os.sched_getaffinity(0))
@@ -575,6 +636,32 @@ def main():
     e2e_ms = max_over_ranks(e2e_ms, world, "cuda")
     e2e_serial_ms = max_over_ranks(e2e_serial_ms, world, "cuda")
 
+    # The link's own ceiling, measured the same way (pinned host memory, the 576 MB SH array in, the 576 MB SH gradient
+    # out): each direction alone, then both at once on two streams.  e2e moves 733 MB each way per step, so
+    # 733 MB / (the both-at-once rate) is the floor of an e2e step on this box whatever the kernels do.
+    def copy_rate(do_in, do_out, reps=3):
+        sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+        t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        t0.record()
+        sa.wait_event(t0); sb.wait_event(t0)
+        for _ in range(reps):
+            if do_in:
+                with torch.cuda.stream(sa):
+                    g["sh"].copy_(host_in["sh"], non_blocking=True)
+            if do_out:
+                with torch.cuda.stream(sb):
+                    host_out["dL_dsh"].copy_(fr.dL_dsh, non_blocking=True)
+        torch.cuda.current_stream().wait_stream(sa)
+        torch.cuda.current_stream().wait_stream(sb)
+        t1.record()
+        torch.cuda.synchronize()
+        return reps * host_in["sh"].numel() * 4 / (t0.elapsed_time(t1) * 1e-3) / 1e9  # GB/s per direction
+
+    link = {"h2d_alone_gb_per_s": round(copy_rate(True, False), 1), "d2h_alone_gb_per_s": round(copy_rate(False, True), 1),
+            "both_at_once_gb_per_s_each_way": round(copy_rate(True, True), 1)}
+    link["floor_ms_per_step"] = round(max(h2d, d2h) / (link["both_at_once_gb_per_s_each_way"] * 1e9) * 1e3, 2)
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -633,6 +720,12 @@ def main():
     if world == 1:
         next_rows = {"mask_head": bench_mask_head(sc, g, hbm_gbs), "inference": bench_inference(sc, g, m),
                      "render_loss": bench_render_loss(sc, hbm_gbs), "optimizer": bench_optimizer(sc, g, fr, hbm_gbs)}
+        ti = bench_training_iteration(sc, g, fr)
+        nr = next_rows
+        ti["sum_of_rows_ms"] = round(ms_step + nr["render_loss"]["ms"] + nr["optimizer"]["ms"]["adam_step"] + nr["optimizer"]["ms"]["density_stats"]
+                                     + sum(nr["mask_head"]["ms"][k] for k in ("mask_sample", "mask_loss", "mask_sample_bwd")), 4)
+        next_rows["training_iteration"] = ti
+        next_rows["training_iteration_ms"] = ti["ms"]
         if args.all_cameras:
             next_rows["all_cameras"] = bench_cameras(sc, g, m)
         if args.config == 3 and not args.no_config5:
@@ -659,7 +752,8 @@ def main():
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": "blends/s", "ms_per_step": e2e_ms, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "how": "pinned host buffers; H2D of all inputs and D2H of image + all gradients every step, software-pipelined over 3 streams and 2 buffer sets",
-                    "ms_per_step_unpipelined": e2e_serial_ms},
+                    "ms_per_step_unpipelined": e2e_serial_ms,
+                    "gb_per_s_each_way": round(max(h2d, d2h) / (e2e_ms * 1e-3) / 1e9, 1), "link_ceiling": link},
             "gpu_launches": launches, "roofline": roofline, "rooflines": rooflines, "cpu_baseline": cpu,
             "next_rows": next_rows}
     print(json.dumps(line), flush=True)

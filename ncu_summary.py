@@ -2,10 +2,15 @@
 traffic per C-ABI call that bench.py prints as `roofline.traffic`.
 
     ncu -i capture.ncu-rep --page raw --csv > raw.csv
-    python -m paper_2412_20522_b200.ncu_summary raw.csv --config 3 --md profiles/r02_ncu_table.md \
-        --traffic-json profiles/r02_traffic.json
+    python ncu_summary.py raw.csv --config 3 --md profiles/r03_ncu_table.md --traffic-json profiles/r03_traffic.json
 
 Reads the CSV only (no GPU, no ncu needed here).  Kernels are attributed to the call of include/mg.h that launches them.
+Measurement tooling: it lives beside bench.py, not in the product package.
+
+Two tables, one row per kernel launch each.  The first is the compute view (time, DRAM bytes, issue and pipe
+utilisation); the second is what north_star asks for on top of it -- shared-memory and L1 data-pipe utilisation against
+peak and bank conflicts for the blend kernels, the `red` (atomic gradient scatter) instruction and sector counts, L1 / L2
+hit rates, and the four largest warp-stall reasons per issued instruction.
 """
 import argparse
 import csv
@@ -22,6 +27,18 @@ COLS = [("Kernel Name", "kernel"), ("gpu__time_duration.sum", "time"), ("dram__b
         ("sm__inst_executed_pipe_xu.avg.pct_of_peak_sustained_active", "xu%"),
         ("lts__throughput.avg.pct_of_peak_sustained_elapsed", "lts%"),
         ("l1tex__throughput.avg.pct_of_peak_sustained_elapsed", "l1tex%")]
+
+# second table: memory pipes, atomics, hit rates (the stall reasons are picked per kernel, see stalls())
+COLS2 = [("Kernel Name", "kernel"),
+         ("l1tex__data_pipe_lsu_wavefronts.avg.pct_of_peak_sustained_elapsed", "lsu_data_pipe%"),
+         ("l1tex__data_pipe_lsu_wavefronts_mem_shared.sum.pct_of_peak_sustained_elapsed", "smem_wavefronts%"),
+         ("l1tex__data_pipe_lsu_wavefronts_mem_shared.sum", "smem_wavefronts"),
+         ("l1tex__data_bank_conflicts_pipe_lsu_mem_shared.sum", "smem_bank_conflicts"),
+         ("smsp__inst_executed_op_global_red.sum", "red_inst"),
+         ("l1tex__t_sectors_pipe_lsu_mem_global_op_red.sum", "red_sectors"),
+         ("lts__d_atomic_input_cycles_active.avg.pct_of_peak_sustained_elapsed", "l2_atomic_unit%"),
+         ("l1tex__t_sector_hit_rate.pct", "l1_hit%"), ("lts__t_sector_hit_rate.pct", "l2_hit%")]
+STALL_PREFIX, STALL_SUFFIX = "smsp__average_warps_issue_stalled_", "_per_issue_active.ratio"
 
 CALL_OF = [("preprocess_bwd", "preprocess_bwd"), ("preprocess_kernel", "preprocess"), ("render_fwd", "render_fwd"),
            ("render_bwd", "render_bwd"), ("depth_keys", "bin_sort"), ("depth_hist", "bin_sort"), ("ctl_", "bin_sort"), ("radix_", "bin_sort"),
@@ -41,6 +58,25 @@ def call_of(kernel):
 
 def short(name):
     return name.replace("<unnamed>::", "").replace("void ", "").split("(")[0][:40]
+
+
+def num(cell):
+    return float(cell.replace(",", ""))
+
+
+def stalls(hdr, r, top=4):
+    """The `top` largest stall reasons of a launch as 'reason value' (warps stalled per issued instruction); `selected`
+    (the warp that did issue) is not a stall and is left out."""
+    out = []
+    for i, h in enumerate(hdr):
+        if h.startswith(STALL_PREFIX) and h.endswith(STALL_SUFFIX) and "not_issued" not in h:
+            name = h[len(STALL_PREFIX):-len(STALL_SUFFIX)]
+            if name != "selected":
+                try:
+                    out.append((num(r[i]), name))
+                except ValueError:
+                    pass
+    return ", ".join(f"{n} {v:.2f}" for v, n in sorted(out, reverse=True)[:top])
 
 
 def main():
@@ -74,6 +110,19 @@ def main():
             b = (float(r[i_rd].replace(",", "")) * UNIT_SCALE[units[i_rd]] + float(r[i_wr].replace(",", "")) * UNIT_SCALE[units[i_wr]])
             traffic[call] = traffic.get(call, 0.0) + b
             time_us[call] = time_us.get(call, 0.0) + float(r[i_t].replace(",", "")) * UNIT_SCALE[units[i_t]]
+    keep2 = [(hdr.index(c), n) for c, n in COLS2 if c in hdr]
+    lines += ["", "Memory pipes, atomics, hit rates and the four largest stall reasons (warps stalled per issued instruction):", "",
+              "| " + " | ".join(n for _, n in keep2) + " | stalls |", "|" + "---|" * (len(keep2) + 1)]
+    for r in body:
+        if len(r) != len(hdr):
+            continue
+        cells = []
+        for i, n in keep2:
+            try:
+                cells.append(f"{num(r[i]):.4g}")
+            except ValueError:
+                cells.append(short(r[i]))
+        lines.append("| " + " | ".join(cells) + " | " + stalls(hdr, r) + " |")
     lines += ["", "Per call (sum over its kernels; time under ncu is cold-cache and serialised):", "",
               "| call | kernels' time (us) | dram read + write (MB) |", "|---|---|---|"]
     for c in ("preprocess", "bin_sort", "render_fwd", "render_bwd", "preprocess_bwd"):

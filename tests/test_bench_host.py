@@ -91,12 +91,12 @@ def test_algorithmic_work_charges_masked_and_unmasked_separately():
 
 def test_roofline_traffic_is_what_the_tracked_ncu_capture_gives(tmp_path):
     """bench.py's `roofline.traffic` comes from profiles/r02_traffic.json; that file must be exactly what
-    paper_2412_20522_b200.ncu_summary derives from the raw ncu CSV tracked beside it (the number was
+    ncu_summary.py (beside bench.py) derives from the raw ncu CSV tracked beside it (the number was
     a constant typed into bench.py and could go stale unnoticed), and every call of the hot path must be in it."""
     root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
     raw = os.path.join(root, "profiles", "r02_ncu_raw.csv")
     out = tmp_path / "traffic.json"
-    subprocess.check_call([sys.executable, "-m", "paper_2412_20522_b200.ncu_summary", raw, "--config", "3",
+    subprocess.check_call([sys.executable, os.path.join(root, "ncu_summary.py"), raw, "--config", "3",
                            "--md", str(tmp_path / "table.md"), "--traffic-json", str(out)], cwd=root)
     derived = json.load(open(out))
     tracked = json.load(open(os.path.join(root, "profiles", "r02_traffic.json")))
@@ -106,6 +106,9 @@ def test_roofline_traffic_is_what_the_tracked_ncu_capture_gives(tmp_path):
     import bench
 
     assert bench.ncu_traffic(3) == tracked["3"]
-    # the table the same script writes has one row per kernel of a step: 22 launches
+    # each of the two tables the same script writes has one row per kernel of a step: 22 launches
     table = open(tmp_path / "table.md").read()
-    assert sum(1 for ln in table.splitlines() if ln.startswith("| ") and "_kernel" in ln) == 22
+    assert sum(1 for ln in table.splitlines() if ln.startswith("| ") and "_kernel" in ln) == 2 * 22
+    # north_star's counters for the blend kernels are in it: shared-memory pipe, bank conflicts, red traffic, stalls
+    bwd = [ln for ln in table.splitlines() if "render_bwd_kernel" in ln]
+    assert len(bwd) == 2 and "short_scoreboard" in bwd[1] and "smem_bank_conflicts" in table and "red_sectors" in table
