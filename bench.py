@@ -300,6 +300,90 @@ def bench_cameras(sc, g, m, steps=10):
             "ms_per_frame_min": float(np.min(ms)), "R_min": min(Rs), "R_max": max(Rs)}
 
 
+def bench_cameras_two_in_flight(sc, g, m, sweeps=3):
+    """The cameras of the scene as INDEPENDENT views (BASELINE.json configs[4]: 20 cameras on a circle; also the
+    inference setting) with two frames in flight: camera k runs on stream k % 2 with its own Frame, so
+    the latency-bound mg_bin_sort and the HBM-bound mg_preprocess of one view run under the issue-bound blend kernels
+    of the other.  A throughput figure over independent views -- never the training-iteration number (an iteration's
+    calls depend on one another).  Timed against the same sweep on one stream, in the same run; every view of the
+    two-stream run is then compared bit for bit (sorted ids, tile ranges, n_contrib, image, final_T) with the
+    sequential one."""
+    import torch
+
+    from paper_2412_20522_b200 import binding as mg
+
+    cams = sc.cameras
+    frs = [mg.Frame(cams[0], sc.N) for _ in range(3)]  # two in flight + one for the sequential sweep
+    Rs = []
+    for cam in cams:
+        frs[0].set_camera(cam)
+        frs[0].preprocess(g)
+        torch.cuda.current_stream().synchronize()
+        Rs.append(int(frs[0].R_host[0]))
+    for f in frs:
+        f.reserve(max(Rs))
+    gimgs = [torch.from_numpy(sc.dL_dimage(ci)).cuda() for ci in range(len(cams))]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    torch.cuda.synchronize()
+
+    def one(fr, ci):
+        fr.set_camera(cams[ci])
+        fr.step(g, m, gimgs[ci])
+
+    def sweep_seq():
+        for ci in range(len(cams)):
+            one(frs[2], ci)
+
+    def sweep_two(first=0, last=None):
+        for ci in range(first, len(cams) if last is None else last):
+            with torch.cuda.stream(streams[ci % 2]):
+                one(frs[ci % 2], ci)
+
+    def join():
+        cur = torch.cuda.current_stream()
+        for st in streams:
+            cur.wait_stream(st)
+
+    sweep_seq(); sweep_two(); join()  # warm-up of both forms
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(sweeps):
+        sweep_seq()
+    e1.record()
+    torch.cuda.synchronize()
+    ms_seq = e0.elapsed_time(e1) / (sweeps * len(cams))
+    e0.record()
+    for st in streams:
+        st.wait_event(e0)
+    for _ in range(sweeps):
+        sweep_two()
+    join()
+    e1.record()
+    torch.cuda.synchronize()
+    ms_two = e0.elapsed_time(e1) / (sweeps * len(cams))
+    # every view, two at a time, against the sequential frame
+    same = True
+    for ci in range(0, len(cams) - 1, 2):
+        sweep_two(ci, ci + 2)
+        join()
+        torch.cuda.synchronize()
+        for k in (0, 1):
+            one(frs[2], ci + k)
+            torch.cuda.synchronize()
+            a, b, R = frs[k], frs[2], Rs[ci + k]
+            same = same and int(a.R_host[1]) == R == int(b.R_host[1])
+            same = same and torch.equal(a.sorted_ids[:R], b.sorted_ids[:R]) and torch.equal(a.tile_ranges, b.tile_ranges)
+            same = same and torch.equal(a.n_contrib, b.n_contrib) and torch.equal(a.image, b.image) and torch.equal(a.final_T, b.final_T)
+    assert same, "two frames in flight changed an output"
+    del frs
+    torch.cuda.empty_cache()
+    return {"ms_per_frame_sequential": round(ms_seq, 4), "ms_per_frame_two_in_flight": round(ms_two, 4),
+            "gain": round(1.0 - ms_two / ms_seq, 4), "frames_timed_each": sweeps * len(cams),
+            "outputs_bit_identical_to_sequential": bool(same),
+            "note": "throughput over independent views on two streams; not a training-iteration figure"}
+
+
 def bench_render_loss(sc, hbm_gbs, reps=30):
     """SURVEY.md 8(f) row f3 at the bench image size.  Algorithmic bytes per image element: 12 (image and target in,
     gradient out); the two-kernel scheme moves 44 (three derivative maps written and read back)."""
@@ -733,6 +817,7 @@ def main():
             sc5 = scenes.make(5)
             g5, m5 = mg.upload(sc5)
             next_rows["config5"] = dict(bench_cameras(sc5, g5, m5, steps=5), workload=workload_name(5).replace(", camera 0", ", its 20 cameras"))
+            next_rows["config5"]["two_in_flight"] = bench_cameras_two_in_flight(sc5, g5, m5)
 
     cpu = None
     if not args.no_cpu_baseline:

@@ -114,6 +114,20 @@ __device__ __forceinline__ unsigned long long ld_relaxed_u64(const unsigned long
   return v;
 }
 
+// ---- programmatic dependent launch (sm_90+).  mg_bin_sort is a chain of 17 short kernels, eight of them 5-16 us
+// long, each of which depends on all of its predecessor: between two such kernels the GPU idles for the launch latency
+// and the drain of the last blocks.  Launched with cudaLaunchAttributeProgrammaticStreamSerialization, a kernel's blocks
+// may become resident while its predecessor is still running; every kernel of this file therefore begins with
+// pdl_prologue(): griddepcontrol.wait blocks until the predecessor grid has COMPLETED and its writes are visible (so
+// nothing of the dependency is given up -- not a load, not a store happens before it, which also covers buffers the
+// predecessor still reads), then griddepcontrol.launch_dependents lets the successor's blocks be scheduled as soon as
+// every block of this grid has started.  What is gained is the launch latency and the tail, nothing else.  Both
+// instructions are no-ops in a kernel launched without the attribute (the first kernel after a memset, MG_NO_PDL).
+__device__ __forceinline__ void pdl_prologue() {
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
+
 constexpr unsigned long long LB_AGGREGATE = 1ull << 32;  // status word = flag << 32 | count
 constexpr unsigned long long LB_INCLUSIVE = 2ull << 32;
 constexpr int LB_SPIN_LIMIT = 1 << 26;                   // polls of one status word before a look-back gives up
@@ -137,6 +151,7 @@ __global__ void __launch_bounds__(RS_THREADS) radix_onesweep_kernel(
     const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in, uint32_t* __restrict__ keys_out,
     uint32_t* __restrict__ vals_out, uint32_t n_all, int pass, SortCtl* __restrict__ ctl,
     unsigned long long* __restrict__ status, int spin_limit) {
+  pdl_prologue();
   extern __shared__ __align__(16) unsigned char rs_smem_raw[];
   RadixSmem& sm = *reinterpret_cast<RadixSmem*>(rs_smem_raw);
   __shared__ uint32_t s_tile, s_nvalid;
@@ -259,6 +274,7 @@ __global__ void __launch_bounds__(RS_THREADS) radix_onesweep_kernel(
 __global__ void __launch_bounds__(256) depth_hist_kernel(int64_t N, const float* __restrict__ depths,
                                                          const uint32_t* __restrict__ tiles_touched,
                                                          SortCtl* __restrict__ ctl) {
+  pdl_prologue();
   __shared__ unsigned long long s_sum[8];
   __shared__ uint32_t s_vis[8];
   __shared__ uint32_t hist[4][RS_BINS];
@@ -300,6 +316,7 @@ __global__ void __launch_bounds__(256) depth_hist_kernel(int64_t N, const float*
 
 // Overflow flag; digit histograms -> exclusive digit bases (one block of 256 threads).
 __global__ void __launch_bounds__(RS_BINS) ctl_finalize_kernel(SortCtl* __restrict__ ctl, unsigned long long capacity) {
+  pdl_prologue();
   __shared__ uint32_t h[4][RS_BINS];
   if (threadIdx.x == 0) ctl->overflow = (ctl->R > capacity || ctl->R >= (1ull << 32)) ? 1u : 0u;
   for (int p = 0; p < 4; p++) h[p][threadIdx.x] = ctl->ghist[p][threadIdx.x];
@@ -331,6 +348,7 @@ __device__ __forceinline__ uint32_t block_reduce_1024(uint32_t v, uint32_t* sh) 
 __global__ void __launch_bounds__(SCAN_THREADS) scan_sums_kernel(const uint32_t* __restrict__ table, uint32_t n_static,
                                                                  const uint32_t* __restrict__ n_dev,
                                                                  uint32_t* __restrict__ sums) {
+  pdl_prologue();
   __shared__ uint32_t sh[32];
   const uint32_t n = scan_n(n_static, n_dev);
   const uint32_t b0 = blockIdx.x * (uint32_t)SCAN_BLK;
@@ -348,6 +366,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) scan_sums_kernel(const uint32_t*
 __global__ void __launch_bounds__(SCAN_THREADS) scan_apply_kernel(uint32_t* __restrict__ table, uint32_t n_static,
                                                                   const uint32_t* __restrict__ n_dev,
                                                                   const uint32_t* __restrict__ sums) {
+  pdl_prologue();
   __shared__ uint32_t sh[32];
   __shared__ uint32_t wsum[32];
   const uint32_t n = scan_n(n_static, n_dev);
@@ -491,6 +510,7 @@ __global__ void __launch_bounds__(32 * XP_MAX_WARPS) row_expand_kernel(
     const uint32_t* __restrict__ order, const int4* __restrict__ rects, const SortCtl* __restrict__ ctl, int gh,
     uint32_t n_chunks, int warps_per_block, uint2* __restrict__ prect, uint32_t* __restrict__ table_r,
     uint2* __restrict__ row_rec) {
+  pdl_prologue();
   extern __shared__ uint32_t xp_smem[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t chunk = blockIdx.x * (uint32_t)warps_per_block + warp;
@@ -552,6 +572,7 @@ __global__ void __launch_bounds__(32 * XP_MAX_WARPS) row_expand_kernel(
 __global__ void __launch_bounds__(1024) plan_kernel(const uint32_t* __restrict__ table_r, uint32_t n_chunks_r, int gh,
                                                     int gw, uint32_t* __restrict__ row_start,
                                                     uint32_t* __restrict__ chunk_base, SortCtl* __restrict__ ctl) {
+  pdl_prologue();
   __shared__ uint32_t part[1024];
   const int per = (gh + 1023) / 1024;
   const int b = threadIdx.x * per, e = min(gh, b + per);
@@ -592,6 +613,7 @@ __global__ void __launch_bounds__(32 * XP_MAX_WARPS) col_expand_kernel(
     const uint2* __restrict__ row_rec, const uint32_t* __restrict__ row_start, const uint32_t* __restrict__ chunk_base,
     const SortCtl* __restrict__ ctl, int gw, int gh, int warps_per_block, uint32_t* __restrict__ table_c,
     uint32_t* __restrict__ sorted_ids) {
+  pdl_prologue();
   extern __shared__ uint32_t xp_smem[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t g = blockIdx.x * (uint32_t)warps_per_block + warp;
@@ -635,6 +657,7 @@ __global__ void __launch_bounds__(256) tile_ranges_kernel(const uint32_t* __rest
                                                           const uint32_t* __restrict__ chunk_base,
                                                           SortCtl* __restrict__ ctl, int gw, int gh,
                                                           uint32_t* __restrict__ tile_ranges) {
+  pdl_prologue();
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
   const int ntiles = gw * gh;
   if (t >= ntiles) return;
@@ -667,6 +690,7 @@ __global__ void __launch_bounds__(256) tile_ranges_kernel(const uint32_t* __rest
 // the atomics give; it affects scheduling only).  Every block rebuilds the 257 class bases in shared memory.
 __global__ void __launch_bounds__(256) tile_order_kernel(const uint32_t* __restrict__ tile_ranges, SortCtl* __restrict__ ctl,
                                                          int ntiles, uint32_t* __restrict__ tile_order) {
+  pdl_prologue();
   __shared__ uint32_t base[TO_CLASSES];
   if (threadIdx.x == 0) {
     uint32_t run = 0;
@@ -725,6 +749,27 @@ inline int xp_warps(int bins) {
   return w;
 }
 
+// Launch `kernel` on `st` so that it may overlap the tail of the kernel before it in the stream (see pdl_prologue).
+template <typename... P, typename... A>
+cudaError_t launch_chained(void (*kernel)(P...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, A... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+#ifdef MG_NO_PDL
+  cfg.attrs = nullptr;
+  cfg.numAttrs = 0;
+#else
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+#endif
+  return cudaLaunchKernelEx(&cfg, kernel, static_cast<P>(args)...);
+}
+
 template <typename K>
 int xp_prepare(K kernel, size_t smem) {
   if (smem > 48 * 1024) MG_CHECK_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -734,8 +779,8 @@ int xp_prepare(K kernel, size_t smem) {
 int scan_table(uint32_t* table, uint32_t n_static, const uint32_t* n_dev, uint32_t n_max, uint32_t* sums, cudaStream_t st) {
   const uint32_t nb = (n_max + SCAN_BLK - 1) / SCAN_BLK;
   const uint32_t grid = nb ? nb : 1;
-  scan_sums_kernel<<<grid, SCAN_THREADS, 0, st>>>(table, n_static, n_dev, sums);
-  scan_apply_kernel<<<grid, SCAN_THREADS, 0, st>>>(table, n_static, n_dev, sums);
+  MG_CHECK_CUDA(launch_chained(scan_sums_kernel, dim3(grid), dim3(SCAN_THREADS), (size_t)(0), st, table, n_static, n_dev, sums));
+  MG_CHECK_CUDA(launch_chained(scan_apply_kernel, dim3(grid), dim3(SCAN_THREADS), (size_t)(0), st, table, n_static, n_dev, sums));
   MG_CHECK_LAUNCH();
   return MG_OK;
 }
@@ -786,7 +831,7 @@ extern "C" int mg_bin_sort(const mg_camera* cam, int64_t N, const float* depths,
   if (N == 0) {
     MG_CHECK_CUDA(cudaMemsetAsync(tile_ranges, 0, sizeof(uint32_t) * 2 * (size_t)gw * gh, st));
     if (tile_order) {
-      tile_order_kernel<<<(gw * gh + 255) / 256, 256, 0, st>>>(tile_ranges, ctl, gw * gh, tile_order);
+      MG_CHECK_CUDA(launch_chained(tile_order_kernel, dim3((gw * gh + 255) / 256), dim3(256), (size_t)(0), st, tile_ranges, ctl, gw * gh, tile_order));
       MG_CHECK_LAUNCH();
     }
     if (R_out_host) MG_CHECK_CUDA(cudaMemcpyAsync(R_out_host, &ctl->R, sizeof(uint64_t), cudaMemcpyDeviceToHost, st));
@@ -811,20 +856,20 @@ extern "C" int mg_bin_sort(const mg_camera* cam, int64_t N, const float* depths,
   MG_CHECK_CUDA(cudaMemsetAsync(status, 0, sizeof(unsigned long long) * 4 * (size_t)L.nblk_sort * RS_BINS, st));
   {
     const int64_t want = (N + 255) / 256;
-    depth_hist_kernel<<<(unsigned)(want < dk_grid ? want : dk_grid), 256, 0, st>>>(N, depths, tiles_touched, ctl);
+    MG_CHECK_CUDA(launch_chained(depth_hist_kernel, dim3((unsigned)(want < dk_grid ? want : dk_grid)), dim3(256), (size_t)(0), st, N, depths, tiles_touched, ctl));
   }
-  ctl_finalize_kernel<<<1, RS_BINS, 0, st>>>(ctl, (unsigned long long)R_capacity);
+  MG_CHECK_CUDA(launch_chained(ctl_finalize_kernel, dim3(1), dim3(RS_BINS), (size_t)(0), st, ctl, (unsigned long long)R_capacity));
   MG_CHECK_LAUNCH();
   {
     // pass 0 reads the caller's depths and tiles_touched and writes the visible (key, index) pairs to B; then B -> A -> B -> A
-    radix_onesweep_kernel<true><<<L.nblk_sort, RS_THREADS, sizeof(RadixSmem), st>>>(
-        reinterpret_cast<const uint32_t*>(depths), tiles_touched, keysB, valsB, (uint32_t)N, 0, ctl, status, spin_limit);
+    MG_CHECK_CUDA(launch_chained(radix_onesweep_kernel<true>, dim3(L.nblk_sort), dim3(RS_THREADS), (size_t)(sizeof(RadixSmem)), st, 
+        reinterpret_cast<const uint32_t*>(depths), tiles_touched, keysB, valsB, (uint32_t)N, 0, ctl, status, spin_limit));
     MG_CHECK_LAUNCH();
     const uint32_t *ki = keysB, *vi = valsB;
     uint32_t *ko = keysA, *vo = valsA;
     for (int pass = 1; pass < 4; pass++) {
-      radix_onesweep_kernel<false><<<L.nblk_sort, RS_THREADS, sizeof(RadixSmem), st>>>(
-          ki, vi, ko, vo, (uint32_t)N, pass, ctl, status + (size_t)pass * L.nblk_sort * RS_BINS, spin_limit);
+      MG_CHECK_CUDA(launch_chained(radix_onesweep_kernel<false>, dim3(L.nblk_sort), dim3(RS_THREADS), (size_t)(sizeof(RadixSmem)), st, 
+          ki, vi, ko, vo, (uint32_t)N, pass, ctl, status + (size_t)pass * L.nblk_sort * RS_BINS, spin_limit));
       MG_CHECK_LAUNCH();
       const uint32_t *tk = ki, *tv = vi;
       ki = ko; vi = vo;
@@ -841,10 +886,10 @@ extern "C" int mg_bin_sort(const mg_camera* cam, int64_t N, const float* depths,
     if (int rc = xp_prepare(row_expand_kernel<false>, smem)) return rc;
     const unsigned grid = (L.n_chunks_r + wpb - 1) / wpb;
     const uint32_t tr = (uint32_t)gh * L.n_chunks_r;
-    row_expand_kernel<true><<<grid, 32 * wpb, smem, st>>>(order, (const int4*)rects, ctl, gh, L.n_chunks_r, wpb, prect, table_r, row_rec);
+    MG_CHECK_CUDA(launch_chained(row_expand_kernel<true>, dim3(grid), dim3(32 * wpb), (size_t)(smem), st, order, (const int4*)rects, ctl, gh, L.n_chunks_r, wpb, prect, table_r, row_rec));
     if (int rc = scan_table(table_r, tr, nullptr, tr, sums, st)) return rc;
-    plan_kernel<<<1, 1024, 0, st>>>(table_r, L.n_chunks_r, gh, gw, row_start, chunk_base, ctl);
-    row_expand_kernel<false><<<grid, 32 * wpb, smem, st>>>(order, (const int4*)rects, ctl, gh, L.n_chunks_r, wpb, prect, table_r, row_rec);
+    MG_CHECK_CUDA(launch_chained(plan_kernel, dim3(1), dim3(1024), (size_t)(0), st, table_r, L.n_chunks_r, gh, gw, row_start, chunk_base, ctl));
+    MG_CHECK_CUDA(launch_chained(row_expand_kernel<false>, dim3(grid), dim3(32 * wpb), (size_t)(smem), st, order, (const int4*)rects, ctl, gh, L.n_chunks_r, wpb, prect, table_r, row_rec));
     MG_CHECK_LAUNCH();
   }
   // S3: column expansion and tile ranges
@@ -855,11 +900,11 @@ extern "C" int mg_bin_sort(const mg_camera* cam, int64_t N, const float* depths,
     if (int rc = xp_prepare(col_expand_kernel<false>, smem)) return rc;
     const unsigned grid = (L.max_chunks_c + wpb - 1) / wpb;
     const uint32_t tc_max = (uint32_t)gw * L.max_chunks_c;
-    col_expand_kernel<true><<<grid, 32 * wpb, smem, st>>>(row_rec, row_start, chunk_base, ctl, gw, gh, wpb, table_c, sorted_ids);
+    MG_CHECK_CUDA(launch_chained(col_expand_kernel<true>, dim3(grid), dim3(32 * wpb), (size_t)(smem), st, row_rec, row_start, chunk_base, ctl, gw, gh, wpb, table_c, sorted_ids));
     if (int rc = scan_table(table_c, 0, &ctl->n_table_c, tc_max, sums, st)) return rc;
-    col_expand_kernel<false><<<grid, 32 * wpb, smem, st>>>(row_rec, row_start, chunk_base, ctl, gw, gh, wpb, table_c, sorted_ids);
-    tile_ranges_kernel<<<(gw * gh + 255) / 256, 256, 0, st>>>(table_c, chunk_base, ctl, gw, gh, tile_ranges);
-    if (tile_order) tile_order_kernel<<<(gw * gh + 255) / 256, 256, 0, st>>>(tile_ranges, ctl, gw * gh, tile_order);
+    MG_CHECK_CUDA(launch_chained(col_expand_kernel<false>, dim3(grid), dim3(32 * wpb), (size_t)(smem), st, row_rec, row_start, chunk_base, ctl, gw, gh, wpb, table_c, sorted_ids));
+    MG_CHECK_CUDA(launch_chained(tile_ranges_kernel, dim3((gw * gh + 255) / 256), dim3(256), (size_t)(0), st, table_c, chunk_base, ctl, gw, gh, tile_ranges));
+    if (tile_order) MG_CHECK_CUDA(launch_chained(tile_order_kernel, dim3((gw * gh + 255) / 256), dim3(256), (size_t)(0), st, tile_ranges, ctl, gw * gh, tile_order));
     MG_CHECK_LAUNCH();
   }
   if (R_out_host) MG_CHECK_CUDA(cudaMemcpyAsync(R_out_host, &ctl->R, sizeof(uint64_t), cudaMemcpyDeviceToHost, st));
