@@ -39,8 +39,8 @@ BYTES_PRE = (301, 109)     # mg_preprocess, per visible / per culled Gaussian
 BYTES_PRE_BWD = (513, 240)  # mg_preprocess_bwd, per visible / per culled Gaussian
 BYTES_SORT_KEY = 22        # mg_bin_sort, per duplicated key, this scheme; the floor of any scheme is 4
 # dram__bytes_read.sum + dram__bytes_write.sum per launch, summed over the kernels of each call: written by
-# `python ncu_summary.py` from the `ncu --set full` capture named in profiles/r02_final.md (section 3)
-TRAFFIC_JSON = os.path.join(ROOT, "profiles", "r02_traffic.json")
+# `python ncu_summary.py` from the `ncu --set full` capture named in profiles/r03_final.md (section 3)
+TRAFFIC_JSON = os.path.join(ROOT, "profiles", "r03_traffic.json")
 # kernels of libmg launched per step (memsets and copies not counted), see binsort.cu for the sort's list
 KERNELS_PER_STEP = {"preprocess": 1, "bin_sort": 2 + 4 + 5 + 6, "render_fwd": 1, "render_bwd": 1,
                     "preprocess_bwd": 2}
@@ -793,7 +793,7 @@ def main():
         dom = max(("render_fwd", "render_bwd"), key=lambda n: per_call[n])
         survey = wc[dom[7:] + "_pair_evals"] * FLOP_PAIR + wc[dom[7:] + "_blends"] * (FLOP_BLEND_BWD if dom == "render_bwd" else FLOP_BLEND_FWD)
         roofline = dict(rooflines[dom], kernel=dom + "_kernel",
-                        traffic_unit="bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum, profiles/r02_final.md)",
+                        traffic_unit="bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum, profiles/r03_final.md)",
                         flop_per_launch=rooflines[dom]["work_per_launch"],
                         flop_counting="masked and unmasked work charged separately (bench.py FLOP_*, DESIGN.md 7.6)",
                         frac_by_survey_constants=survey / (per_call[dom] * 1e-3) / 1e12 / fp32_peak,

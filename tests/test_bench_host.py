@@ -90,16 +90,16 @@ def test_algorithmic_work_charges_masked_and_unmasked_separately():
 
 
 def test_roofline_traffic_is_what_the_tracked_ncu_capture_gives(tmp_path):
-    """bench.py's `roofline.traffic` comes from profiles/r02_traffic.json; that file must be exactly what
+    """bench.py's `roofline.traffic` comes from profiles/r03_traffic.json; that file must be exactly what
     ncu_summary.py (beside bench.py) derives from the raw ncu CSV tracked beside it (the number was
     a constant typed into bench.py and could go stale unnoticed), and every call of the hot path must be in it."""
     root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-    raw = os.path.join(root, "profiles", "r02_ncu_raw.csv")
+    raw = os.path.join(root, "profiles", "r03_ncu_raw.csv")
     out = tmp_path / "traffic.json"
     subprocess.check_call([sys.executable, os.path.join(root, "ncu_summary.py"), raw, "--config", "3",
                            "--md", str(tmp_path / "table.md"), "--traffic-json", str(out)], cwd=root)
     derived = json.load(open(out))
-    tracked = json.load(open(os.path.join(root, "profiles", "r02_traffic.json")))
+    tracked = json.load(open(os.path.join(root, "profiles", "r03_traffic.json")))
     assert derived == tracked
     assert set(tracked["3"]) == {"preprocess", "bin_sort", "render_fwd", "render_bwd", "preprocess_bwd"}
     sys.path.insert(0, root)
